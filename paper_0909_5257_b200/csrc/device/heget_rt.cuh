@@ -1,0 +1,101 @@
+// heget-b200: run-time support shared by every generated per-process kernel file (gen_*.cu) and by the C-ABI (api.cpp).
+//
+// A generated file defines, for one process, the kernels of steps a3-a8 (eq. 4), a host
+// launcher and a static descriptor which it registers with the library at load time.  Nothing here is process specific.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "heget_dev.cuh"
+
+namespace hg {
+
+// ---- descriptor of one generated process (host side) -------------------------------------------------------------------
+struct LaunchArgs {
+    const double* d_mom;      // [n_ext][4][n_events] FP64, device
+    uint64_t n_events;
+    double inv_sqrt_s;        // momenta are evaluated in units of sqrt(s_hat) (reading A21)
+    double out_scale;         // S * 1/4 * 1/(n_a n_b) * g^(2(n-2)) * s_hat^-(n-4)      (eqs. 4, 9, 12)
+    void* d_me2;              // double[n_events] or float[n_events]
+    int hel_mode;             // 0 = sum over all helicities, 1 = one Philox-drawn helicity per event, 2 = fixed configuration
+    int hel_fixed;            // mode 2: index of the configuration in the kernel's own enumeration, or -1 (vanishing)
+    uint64_t seed;            // mode 1
+    uint64_t first_event;     // mode 1: global index of event 0 (Philox counter)
+    void* d_jbuf;             // colour-GEMM variant: J chunk [2*NJ][columns], else NULL
+    int lanes;                // helicity lanes per event (power of two <= 32), 0 = choose
+    cudaStream_t stream;
+};
+
+struct KernelInfo { int regs, local_bytes, smem_static, max_threads; };
+
+struct ProcDesc {
+    const char* name;           // canonical process string, e.g. "g g > g g g"
+    const char* tag;
+    int n_ext, n_gluons, n_quark_legs;
+    int n_hel;                  // 2^n_ext, the helicity configurations of eq. 12
+    int n_hel_eval;             // configurations that are not identically zero (quark-line chirality conservation)
+    int n_diagrams;             // paper's convention: a four-gluon vertex counts 3 (Table 1)
+    int n_topologies;
+    int n_currents;             // distinct off-shell sub-currents per helicity configuration
+    int n_color;                // colour basis in the paper's convention (Table 1)
+    int n_color_eval;           // basis the kernel sums diagrams on
+    int n_color_reduced;        // after merging elements whose J are proportional
+    double sym_factor, avg_color, avg_spin;
+    double flops_per_hel;       // counted from the generator's IR (per evaluated helicity configuration)
+    double flops_per_event;     // prologue + n_hel_eval * flops_per_hel
+    double flops_colour_per_hel;
+    const double* colour_matrix;        // n_color x n_color, paper basis, without 1/(n_a n_b)  (eq. 9)
+    const double* colour_matrix_eval;   // n_color_reduced x n_color_reduced
+    const signed char* hel_table;       // [n_hel_eval][n_ext] physical helicities of the kernel's enumeration
+    int (*launch)(int prec, const LaunchArgs&);                 // returns cudaError_t
+    int (*kernel_info)(int prec, int lanes, KernelInfo*);       // registers / local memory of the compiled kernel
+    int block[2];               // threads per block, FP64 / FP32
+    ProcDesc* next;
+};
+
+void register_process(ProcDesc* d);     // defined in api.cpp
+ProcDesc* registry_head();
+
+struct Registrar { explicit Registrar(ProcDesc* d) { register_process(d); } };
+
+#if defined(HG_HOST_DEBUG)
+#define HG_SMEM_DECL static unsigned char hg_smem[1 << 20]
+#else
+#define HG_SMEM_DECL extern __shared__ __align__(16) unsigned char hg_smem[]
+#endif
+#if defined(__CUDACC__) || defined(HG_HOST_DEBUG)
+// ---- device helpers used by the generated code ------------------------------------------------------------------------
+template <typename T> __device__ __forceinline__ mom4<T> ldk(const T* ev, int slot, int stride) {
+    mom4<T> k;
+    k.p[0] = ev[(slot + 0) * stride]; k.p[1] = ev[(slot + 1) * stride]; k.p[2] = ev[(slot + 2) * stride]; k.p[3] = ev[(slot + 3) * stride];
+    return k;
+}
+template <typename T> __device__ __forceinline__ vec4<T> ldv(const T* ev, int slot, int stride, T lambda) {   // vxxxxx, helicity part
+    vec4<T> w;
+    w.v[0] = mk<T>(T(0), T(0));
+    w.v[1] = mk<T>(lambda * ev[(slot + 0) * stride], ev[(slot + 3) * stride]);
+    w.v[2] = mk<T>(lambda * ev[(slot + 1) * stride], ev[(slot + 4) * stride]);
+    w.v[3] = mk<T>(lambda * ev[(slot + 2) * stride], ev[(slot + 5) * stride]);
+    return w;
+}
+template <typename T> __device__ __forceinline__ sp2<T> ldi(const T* ev, int slot, int stride, T chi) {       // ixxxxx, helicity part
+    const T s[3] = {ev[slot * stride], ev[(slot + 1) * stride], ev[(slot + 2) * stride]};
+    return ixxxxx<T>(s, chi);
+}
+template <typename T> __device__ __forceinline__ sp2<T> ldo(const T* ev, int slot, int stride, T chi) {       // oxxxxx, helicity part
+    const T s[3] = {ev[slot * stride], ev[(slot + 1) * stride], ev[(slot + 2) * stride]};
+    return oxxxxx<T>(s, chi);
+}
+
+// Philox4x32-10 (Salmon et al., SC'11): the counter-based generator of steps a1 and of HEL_SAMPLE (reading A17)
+__host__ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t* out) {
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+#endif
+
+}  // namespace hg

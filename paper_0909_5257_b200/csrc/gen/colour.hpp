@@ -206,10 +206,11 @@ struct ColourAlgebra {
         return contract(e, b, keep_bridge);
     }
     // the three colour structures of the four-gluon vertex (eq. 40), open index d:
-    //   piece 0: f^{abe}f^{cde}   piece 1: f^{ace}f^{bde}   piece 2: f^{ade}f^{bce}
+    //   piece 0: f^{abe}f^{cde}   piece 1: f^{ace}f^{dbe}   piece 2: f^{ade}f^{bce}
+    // (i f^{abe})(i f^{ecd}) = -f^{abe}f^{cde};  (i f^{ace})(i f^{ebd}) = +f^{ace}f^{dbe};  (i f^{bce})(i f^{aed}) = +f^{ade}f^{bce}
     CExpr join4(const CExpr& X, const CExpr& Y, const CExpr& Z, int piece) {
         if (piece == 0) return scaled(join3(join3(X, Y), Z), Frac(-1));
-        if (piece == 1) return scaled(join3(join3(X, Z), Y), Frac(-1));
+        if (piece == 1) return join3(join3(X, Z), Y);
         return join3(X, join3(Y, Z));
     }
     // quark + gluon -> quark, colour factor -T^a_{ij} (eq. 22): the generator goes on the open end
