@@ -1,0 +1,137 @@
+/* heget-b200: C-ABI of the hot path of arxiv 0909.5257 ("Calculation of QCD processes on GPU"), built for NVIDIA B200.
+ *
+ * What the path computes (eq. 4; eqs. 7-12): for each phase-space point the helicity-summed,
+ * colour-summed and averaged tree-level squared matrix element of a massless-QCD n-jet subprocess
+ *
+ *      me2 = S * 1/4 * 1/(n_a n_b) * sum_lambda  sum_{alpha,beta} J_alpha^* C_{alpha beta} J_beta ,
+ *      J_alpha = sum_l c_{alpha l} A_l(lambda)                       (eqs. 8-10)
+ *
+ * where A_l are the HELAS-style diagram amplitudes built from ixxxxx/oxxxxx/vxxxxx wavefunctions and the qqg, ggg, gggg
+ * vertex functions of the paper's section 4, C is the real symmetric colour matrix of eq. 9, S the
+ * identical-particle factor, 1/4 the spin average (eq. 12) and 1/(n_a n_b) the colour average (eq. 9).
+ *
+ * Conventions shared by every entry point
+ *   - plain C, no exceptions cross the boundary; every function that can fail returns heget_status_t and leaves a
+ *     message retrievable with heget_last_error() (thread-local);
+ *   - pointers named d_* are DEVICE pointers owned by the caller (e.g. torch tensors), pointers named h_* are HOST
+ *     pointers owned by the caller; the library never frees or reallocates them;
+ *   - work is enqueued asynchronously on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ *     stream); the d_* entry points do not synchronise.  The h_* ("host buffer") entry points copy in/out on that
+ *     stream and synchronise it before returning;
+ *   - momenta are always FP64, laid out structure-of-arrays  mom[(leg*4 + mu)*n_events + e],  mu = (E, px, py, pz) in GeV,
+ *     legs = the two initial partons followed by the finals in process-string order;
+ *   - there is no CPU fallback: without a CUDA device the compute entry points return HEGET_ECUDA.
+ */
+#ifndef HEGET_H
+#define HEGET_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct heget_process heget_process_t;      /* opaque; created by heget_process_create, freed by heget_destroy */
+
+typedef enum {
+    HEGET_OK = 0,
+    HEGET_EINVAL = 1,        /* NULL handle / NULL required pointer / malformed argument                       */
+    HEGET_EUNSUPPORTED = 2,  /* a syntactically valid process outside massless QCD {g, u, u~}, or too large     */
+    HEGET_ECUDA = 3,         /* a CUDA runtime call failed (message holds cudaGetErrorString)                   */
+    HEGET_ENOMEM = 4,
+    HEGET_ECOMPILE = 5       /* no pre-built kernel for the process and run-time generation/compilation failed  */
+} heget_status_t;
+
+typedef enum { HEGET_FP64 = 0, HEGET_FP32 = 1 } heget_precision_t;
+
+/* helicity treatment of eq. 12.  SUM: all 2^n_ext configurations (the graded mode, reading A8).
+ * SAMPLE: one configuration per event drawn from Philox(seed, global event index), weighted by 2^n_ext -- what the paper
+ * itself ran.  FIXED: the single configuration given in `hel` (no weight). */
+typedef enum { HEGET_HEL_SUM = 0, HEGET_HEL_SAMPLE = 1, HEGET_HEL_FIXED = 2 } heget_hel_mode_t;
+
+/* jet cuts in the partonic centre-of-mass frame (eqs. 14a, 14b, 15b; reading A9): pT > pt_min [GeV],
+ * |eta| < eta_max, Delta R_ij > dr_min for every final pair; a value <= 0 disables that cut. */
+typedef struct { double pt_min, eta_max, dr_min; } heget_cuts_t;
+
+typedef struct {
+    int n_ext;                 /* external legs                                                                  */
+    int n_hel;                 /* 2^n_ext helicity configurations of eq. 12                                       */
+    int n_hel_eval;            /* of which not identically zero (massless quark lines conserve chirality)         */
+    int n_diagrams;            /* Table 1 convention: a four-gluon vertex counts three times    */
+    int n_topologies;          /* plain Feynman-diagram topologies                                                */
+    int n_color;               /* colour-basis size in the paper's convention (Table 1)                           */
+    int n_color_eval;          /* size of the basis the kernel accumulates J on                                   */
+    int n_color_reduced;       /* after merging elements whose J are proportional for every phase-space point     */
+    double avg_spin;           /* 1/4                       (eq. 12)                                              */
+    double avg_color;          /* 1/(n_a n_b)               (eq. 9)                                               */
+    double sym_factor;         /* 1/prod k!                                         */
+    double flops_per_event;    /* counted by the generator from the code it emitted, HEL_SUM, FMA = 2             */
+    double flops_per_helicity;
+    int regs_per_thread;       /* of the kernel HEL_SUM launches at large n_events, this precision                */
+    int local_bytes_per_thread;/* stack frame (spills) of the same kernel; 0 = everything stays in registers      */
+    int threads_per_block;
+} heget_info_t;
+
+/* Build (or look up) the specialised kernels of one process.
+ *   process     "u u~ > g g", "g g > g g g", ...: two initial and >= 2 final partons out of {g, u, u~}   (eq. 3/13)
+ *   sqrt_s_hat  partonic centre-of-mass energy in GeV (> 0)                                              (eq. 2)
+ *   alpha_s     fixed strong coupling (> 0); g_s = sqrt(4 pi alpha_s)
+ *   cuts        may be NULL (no cuts)
+ *   out         receives the handle on HEGET_OK; untouched otherwise
+ * The kernels of a process come from the pre-built plug-in paper_0909_5257_b200/kernels/heget_<tag>.so if it exists;
+ * otherwise the generator runs in-process, nvcc compiles its output for sm_100a and the result is cached there
+ * (HEGET_ECOMPILE if nvcc is missing or fails).  Synchronous. */
+heget_status_t heget_process_create(const char* process, double sqrt_s_hat, double alpha_s, const heget_cuts_t* cuts,
+                                    heget_precision_t prec, heget_process_t** out);
+
+heget_status_t heget_process_info(const heget_process_t* proc, heget_info_t* out);
+
+/* Colour matrix C of eq. 9 WITHOUT the 1/(n_a n_b) average, row-major.
+ *   which = 0: n_color x n_color in the paper's basis (Tables 1 and 4);  which = 1: the reduced matrix the kernel contracts.
+ * h_out may be NULL to query the dimension only; *n receives the dimension. */
+heget_status_t heget_color_matrix(const heget_process_t* proc, int which, double* h_out, int* n);
+
+/* Steps a1-a2: Philox4x32-10 uniforms -> massless RAMBO momenta in the partonic CM frame -> cuts, re-drawing a failed
+ * event with attempt = 0, 1, 2, ... (cap 65536; then weight 0) (readings A7, A9, A17, A18).
+ * Event e of this call is global event first_event + e: the result does not depend on how events are sharded.
+ *   d_mom     double[n_ext*4*n_events]   required
+ *   d_weight  double[n_events] or NULL   flat phase-space weight of the accepted point (0 if the cap was hit)
+ *   d_tries   uint32[n_events] or NULL   attempts used
+ * n_events == 0 is a no-op returning HEGET_OK. */
+heget_status_t heget_sample_momenta(heget_process_t* proc, uint64_t seed, uint64_t first_event, uint64_t n_events,
+                                    double* d_mom, double* d_weight, uint32_t* d_tries, void* cuda_stream);
+
+/* Steps a3-a8: me2[e] of eq. 4 for every event.
+ *   d_mom   double[n_ext*4*n_events] as written by heget_sample_momenta (any on-shell massless momenta with
+ *           p_a + p_b = sum p_final are accepted)
+ *   mode    see heget_hel_mode_t;  hel = n_ext entries of +-1 (host pointer) for FIXED, else ignored;
+ *           seed/first_event only matter for SAMPLE
+ *   d_me2   double[n_events] (HEGET_FP64 handle) or float[n_events] (HEGET_FP32 handle)
+ * n_events == 0 is a no-op returning HEGET_OK. */
+heget_status_t heget_eval_me2(heget_process_t* proc, const double* d_mom, uint64_t n_events, heget_hel_mode_t mode,
+                              const int8_t* hel, uint64_t seed, uint64_t first_event, void* d_me2, void* cuda_stream);
+
+/* The same two steps with HOST buffers: the library stages through a device scratch it owns (grown on demand, freed by
+ * heget_destroy), copies on `cuda_stream` and synchronises it before returning.  h_me2 is double[] or float[] per the
+ * handle's precision.  Either of h_mom_in / h_mom_out may be NULL:
+ *   heget_run_host(.., h_mom_in = NULL, ..)  samples (seed, first_event) on the device, evaluates, returns me2 (and the
+ *                                            momenta / weights if h_mom_out / h_weight are non-NULL);
+ *   heget_run_host(.., h_mom_in != NULL, ..) uploads the given momenta and evaluates them. */
+heget_status_t heget_run_host(heget_process_t* proc, uint64_t seed, uint64_t first_event, uint64_t n_events,
+                              const double* h_mom_in, double* h_mom_out, double* h_weight, heget_hel_mode_t mode,
+                              const int8_t* hel, void* h_me2, void* cuda_stream);
+
+/* Choose the number of helicity lanes per event for HEL_SUM (a power of two the kernel was built with, or 0 = automatic:
+ * several lanes per event for small batches, one event per thread for large ones). */
+heget_status_t heget_set_lanes(heget_process_t* proc, int lanes);
+
+void heget_destroy(heget_process_t* proc);          /* NULL is allowed */
+
+const char* heget_last_error(void);                 /* thread-local, valid until the next call on this thread */
+
+/* number of kernel launches this library has enqueued since it was loaded (bench.py's gpu_launches) */
+uint64_t heget_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HEGET_H */

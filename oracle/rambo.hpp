@@ -11,6 +11,8 @@
 //      Q = sum q, M = sqrt(Q^2), b = -Q_vec/M, x = sqrt(s_hat)/M, gamma = Q0/M, a = 1/(1+gamma)
 //        p0 = x (gamma q0 + b.q),  p_vec = x (q_vec + b q0 + a (b.q) b)
 //      weight w0 = (pi/2)^(n-1) s_hat^(n-2) / ((n-1)! (n-2)!) (2 pi)^(4-3n)
+//  A7b after the boost the point is put back on the constraint surface (see rambo_attempt): floating-point RAMBO
+//      misses momentum conservation by eps Q0^2/M^2, which reaches 1e-10 among 10^4 two-body events
 //  A17 Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): multipliers 0xD2511F53, 0xCD9E8D57, Weyl key
 //      increments 0x9E3779B9, 0xBB67AE85, 10 rounds; counter = (event_lo, event_hi, attempt, particle),
 //      key = (seed_lo, seed_hi); uniform u = (k + 0.5) 2^-32.
@@ -97,6 +99,20 @@ inline void rambo_attempt(int n, double sqrt_s, uint64_t seed, uint64_t event, u
         p[i][0] = x * (gamma * q[i][0] + bq);
         for (int k = 0; k < 3; ++k) p[i][1 + k] = x * (q[i][1 + k] + b[k] * q[i][0] + a * bq * b[k]);
     }
+    // A7b: the boost above forms each p_i from terms gamma^2 times larger than the result (gamma = Q0/M), so in
+    // floating point sum p_i misses (sqrt_s, 0, 0, 0) by ~ eps gamma^2 sqrt_s, and gamma^2 has a 1/G tail for n = 2.
+    // The point is put back on the constraint surface: remove the residual 3-momentum evenly, set E_i = |p_i|
+    // (exactly massless), rescale to sum E_i = sqrt_s.  The shift is of the size of the rounding error it removes.
+    double d[3] = {0, 0, 0};
+    for (int i = 0; i < n; ++i) for (int k = 0; k < 3; ++k) d[k] += p[i][1 + k];
+    double Et = 0;
+    for (int i = 0; i < n; ++i) {
+        for (int k = 0; k < 3; ++k) p[i][1 + k] -= d[k] / (double)n;
+        p[i][0] = std::sqrt(p[i][1] * p[i][1] + p[i][2] * p[i][2] + p[i][3] * p[i][3]);
+        Et += p[i][0];
+    }
+    const double r = sqrt_s / Et;
+    for (int i = 0; i < n; ++i) for (int m = 0; m < 4; ++m) p[i][m] *= r;
 }
 
 inline double rambo_flat_weight(int n, double sqrt_s) {

@@ -1,7 +1,7 @@
 // heget-b200: run-time support shared by every generated per-process kernel file (gen_*.cu) and by the C-ABI (api.cpp).
 //
 // A generated file defines, for one process, the kernels of steps a3-a8 (eq. 4), a host
-// launcher and a static descriptor which it registers with the library at load time.  Nothing here is process specific.
+// launcher and a static descriptor which the library reads through heget_plugin_desc() after dlopen.  Nothing here is process specific.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -52,10 +52,7 @@ struct ProcDesc {
     ProcDesc* next;
 };
 
-void register_process(ProcDesc* d);     // defined in api.cpp
-ProcDesc* registry_head();
-
-struct Registrar { explicit Registrar(ProcDesc* d) { register_process(d); } };
+// every plug-in (one shared object per process) exports   extern "C" const hg::ProcDesc* heget_plugin_desc();
 
 #if defined(HG_HOST_DEBUG)
 #define HG_SMEM_DECL static unsigned char hg_smem[1 << 20]
