@@ -1,0 +1,287 @@
+"""bench.py -- events/s of the whole hot path (Philox+RAMBO+cuts -> helicity- and colour-summed |M|^2) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--precision fp64] [--impl ours|reference]
+
+One "step" = one pass of steps a1-a8 over one batch of E synthetic events: heget_sample_momenta then
+heget_eval_me2 on device-resident buffers.  Default workload: BASELINE.json configs[1] = C2, g g -> g g g, 2^20 events,
+sqrt(s_hat) = 1 TeV, FP64.  Prints ONE JSON line (rank 0).  N > 1: one process per GPU under torchrun, every rank takes
+E events of its own global range (weak scaling, no collective on the data path).
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+CONFIGS = {   # BASELINE.json configs / SURVEY.md 8 table: process, sqrt(s_hat) [GeV], events, Philox seed
+    "C1": ("u u~ > g g", 500.0, 1 << 14, 0),
+    "C2": ("g g > g g g", 1000.0, 1 << 20, 1),
+    "C3": ("u u > u u g g", 1000.0, 1 << 20, 2),
+    "C4": ("g g > g g g g", 1500.0, 1 << 20, 3),
+    "C5": ("u u~ > g g g g g", 2000.0, 1 << 18, 4),
+}
+ORACLE_SAMPLE = {"C1": 1 << 14, "C2": 1 << 15, "C3": 1 << 13, "C4": 1 << 10, "C5": 1 << 7}   # ~10-30 s of host work
+METRIC = "helicity-summed |M|^2 events/sec per process on 1 B200; % of FP64/FP32 peak"
+SM_COUNT, FP64_LANES, FP32_LANES = 148, 64, 128      # per SM; DESIGN.md "Roofline" derives the ALU peak from these
+
+
+def peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks line of /opt/skills/guides/B200_PROFILING.md, sampled during the timed region."""
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + q, "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, reasons, mx, pw = [], set(), None, []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1]); pw.append(float(r[2]))
+                for k, nm in enumerate(names):
+                    if r[3 + k].strip().lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        if sm:
+            hi = [x for x in sm if x >= 0.5 * max(sm)]
+            out = {"sm_mhz": statistics.median(hi), "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm),
+                   "power_w_max": max(pw) if pw else None}
+        return out
+
+
+def run_reference(a):
+    """The CPU oracle, as it stands, on a bounded sample of the workload (host cores of this box)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    name, sqrt_s, E, seed = CONFIGS[a.config]
+    n = min(E, ORACLE_SAMPLE[a.config])
+    P = O.Process(name, 0.118)
+    nf = P.n_ext - 2
+    times = []
+    for k in range(a.warmup + a.steps):
+        t0 = time.perf_counter()
+        mom, w, tr = O.sample_momenta(nf, sqrt_s, seed, n, first_event=k * n)
+        me2 = P.me2(mom)
+        dt = time.perf_counter() - t0
+        if k >= a.warmup:
+            times.append(dt)
+    assert me2.min() > 0
+    tot = sum(times)
+    v = n * len(times) / tot
+    cores = O.max_threads()
+    sample = "%d of %d events per step (first events of the seed-%d stream), FP64, OpenMP over events" % (n, E, seed)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": "events/s", "n_gpus": a.gpus, "steps": a.steps, "warmup": a.warmup,
+        "ms_per_step": 1e3 * tot / len(times), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "%s: %s, sqrt_s_hat=%g GeV, %d events/step" % (a.config, name, sqrt_s, E), "precision": "fp64"},
+        "cpu_baseline": {"value": v, "unit": "events/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def run_ours(a):
+    import torch
+    import torch.distributed as dist
+    import paper_0909_5257_b200 as hg
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    name, sqrt_s, E, seed = CONFIGS[a.config]
+    P = hg.Process(name, sqrt_s, precision=a.precision)
+    info = P.info
+    ne = info.n_ext
+    first = rank * E                      # weak scaling: rank r evaluates global events [rE, (r+1)E)
+    mom = torch.empty(ne, 4, E, dtype=torch.float64, device="cuda")
+    wgt = torch.empty(E, dtype=torch.float64, device="cuda")
+    me2 = torch.empty(E, dtype=P.dtype, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    need_flush = mom.numel() * 8 < (160 << 20)
+
+    def step(k):
+        P.sample_momenta(seed, E, first_event=first + k * world * E, mom=mom, weight=wgt)
+        P.eval_me2(mom, out=me2)
+
+    # ---- device-resident throughput: K steps between two events, barrier + synchronize on both sides ---------------------
+    for k in range(a.warmup):
+        step(k)
+    barrier()
+    clocks = ClockSampler(local) if rank == 0 else None
+    c0 = hg.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * a.steps)]
+    for k in range(a.steps):
+        if need_flush:
+            flush.fill_(k & 0xff)
+        ev[2 * k].record()
+        step(a.warmup + k)
+        ev[2 * k + 1].record()
+    barrier()
+    launches = hg.launch_count() - c0
+    ms = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(a.steps))
+    ms = max_over_ranks(ms)
+    clk = clocks.stop() if clocks else None
+    value = world * E * a.steps / (ms * 1e-3)
+    assert bool(torch.isfinite(me2).all()) and float(me2.min()) > 0.0
+
+    # ---- the dominant kernel alone (heget_eval_me2), for the roofline --------------------------------------------------
+    kev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * a.steps)]
+    for k in range(a.steps):
+        if need_flush:
+            flush.fill_(k & 0xff)
+        kev[2 * k].record()
+        P.eval_me2(mom, out=me2)
+        kev[2 * k + 1].record()
+    torch.cuda.synchronize()
+    k_ms = sum(kev[2 * k].elapsed_time(kev[2 * k + 1]) for k in range(a.steps)) / a.steps
+    sev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    sev[0].record()
+    for k in range(a.steps):
+        P.sample_momenta(seed, E, first_event=first, mom=mom, weight=wgt)
+    sev[1].record()
+    torch.cuda.synchronize()
+    s_ms = sev[0].elapsed_time(sev[1]) / a.steps
+    achieved = info.flops_per_event * E / (k_ms * 1e-3) / 1e12
+    pk = peaks()
+    sm_max = float(pk.get("sm_max_mhz", 1965.0))
+    lanes = FP64_LANES if a.precision == "fp64" else FP32_LANES
+    peak = SM_COUNT * lanes * 2 * sm_max * 1e6 / 1e12
+    # measured FMA-chain peak of this GPU at the clock it holds under this kind of load
+    prec = hg.FP64 if a.precision == "fp64" else hg.FP32
+    nthr = SM_COUNT * 2048
+    hg.fma_probe(prec, 1 << 12, nthr)
+    torch.cuda.synchronize()
+    pev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    pev[0].record()
+    fl = hg.fma_probe(prec, 1 << 16, nthr)
+    pev[1].record()
+    torch.cuda.synchronize()
+    probe = fl / (pev[0].elapsed_time(pev[1]) * 1e-3) / 1e12
+
+    # ---- end to end through the C-ABI with HOST buffers ----------------------------------------------------------------
+    h_mom = torch.empty(ne, 4, E, dtype=torch.float64).pin_memory()
+    h_me2 = torch.empty(E, dtype=P.dtype).pin_memory()
+    h_mom.copy_(mom)
+    for k in range(2):
+        P.run_host(seed, E, mom_in=h_mom, out=h_me2)
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(a.steps):
+        P.run_host(seed, E, mom_in=h_mom, out=h_me2)
+    barrier()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e = world * E * a.steps / e2e_s
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- CPU oracle on a bounded sample (N = 1 only) -------------------------------------------------------------------
+    cpu = None
+    if world == 1 and not a.no_cpu_baseline:
+        from oracle import oracle as O
+        n = min(E, ORACLE_SAMPLE[a.config])
+        Po = O.Process(name, 0.118)
+        t0 = time.perf_counter()
+        m_o, _, _ = O.sample_momenta(ne - 2, sqrt_s, seed, n)
+        r_o = Po.me2(m_o)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n / dt, "unit": "events/s", "cores": O.max_threads(), "kind": "oracle",
+               "sample": "first %d of the %d seed-%d events, FP64, OpenMP over events, %.1f s" % (n, E, seed, dt)}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+        "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if a.precision == "fp64" else "f32", "data": "synthetic",
+        "config": {"workload": "%s: %s, sqrt_s_hat=%g GeV, %d events/step/GPU, Philox seed %d, cuts pT>20 |eta|<2.5 dR>0.4, full %d-helicity sum"
+                               % (a.config, name, sqrt_s, E, seed, info.n_hel),
+                   "precision": a.precision, "l2": "flushed between steps" if need_flush else "inputs larger than L2 (%d MiB momenta)" % (mom.numel() * 8 >> 20),
+                   "parallelism": "events sharded over %d GPU(s), no collective" % world},
+        "roofline": {"bound": "alu", "kernel": "heget_eval_me2 (%d-thread blocks, %d regs, %d B local)" % (info.threads_per_block, info.regs_per_thread, info.local_bytes_per_thread),
+                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                     "peak_kind": "nominal %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md)" % (SM_COUNT, lanes, sm_max),
+                     "fma_probe_tflops": probe, "frac_of_probe": achieved / probe,
+                     "flops_per_event": info.flops_per_event, "kernel_ms": k_ms, "sampling_kernel_ms": s_ms,
+                     "kernel_share_of_step": k_ms / (ms / a.steps)},
+        "cpu_baseline": cpu,
+        "e2e": {"value": e2e, "unit": "events/s", "h2d_bytes_per_step": int(h_mom.numel() * 8), "d2h_bytes_per_step": int(h_me2.numel() * h_me2.element_size()),
+                "what": "heget_run_host: pinned host momenta -> device, heget_eval_me2, me2 -> pinned host, stream synchronised, per step"},
+        "gpu_launches": int(launches), "clocks": clk,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2", choices=sorted(CONFIGS))
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    a = ap.parse_args()
+    a.warmup = max(a.warmup, 3) if a.impl == "ours" else a.warmup
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
+
+
+if __name__ == "__main__":
+    main()

@@ -128,6 +128,13 @@ void heget_destroy(heget_process_t* proc);          /* NULL is allowed */
 
 const char* heget_last_error(void);                 /* thread-local, valid until the next call on this thread */
 
+/* Measurement aid for the ALU roofline: n_threads threads (a multiple of 256) each run 8 independent
+ * register-resident chains of `iters` dependent FMAs in the given precision; *flops receives the flops enqueued
+ * (16 * iters * n_threads).  d_out: device array of n_threads elements of that precision.  Not part of the hot path and
+ * not counted by heget_launch_count. */
+heget_status_t heget_fma_probe(heget_precision_t prec, uint64_t iters, void* d_out, uint64_t n_threads, double* flops,
+                               void* cuda_stream);
+
 /* number of kernel launches this library has enqueued since it was loaded (bench.py's gpu_launches) */
 uint64_t heget_launch_count(void);
 

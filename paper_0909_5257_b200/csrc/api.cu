@@ -111,6 +111,17 @@ double rambo_flat_weight(int n, double sqrt_s) {      // reading A7: (pi/2)^(n-1
     return w;
 }
 
+// register-resident chains of dependent FMAs, 8 independent chains per thread: the measured vector-FP peak of 8(d)
+template <typename T>
+__global__ void __launch_bounds__(256) k_fma_probe(T* out, unsigned long long iters, T a, T b) {
+    T x0 = T(threadIdx.x), x1 = x0 + T(1), x2 = x0 + T(2), x3 = x0 + T(3), x4 = x0 + T(4), x5 = x0 + T(5), x6 = x0 + T(6), x7 = x0 + T(7);
+    for (unsigned long long i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
 }  // namespace
 
 struct heget_process {
@@ -126,6 +137,17 @@ extern "C" {
 
 const char* heget_last_error(void) { return g_err; }
 uint64_t heget_launch_count(void) { return g_launches.load(); }
+
+heget_status_t heget_fma_probe(heget_precision_t prec, uint64_t iters, void* d_out, uint64_t n_threads, double* flops, void* cuda_stream) {
+    if (!d_out || !flops || n_threads == 0 || n_threads % 256) return fail(HEGET_EINVAL, "heget_fma_probe: d_out/flops NULL or n_threads not a multiple of 256");
+    const unsigned int blocks = (unsigned int)(n_threads / 256);
+    if (prec == HEGET_FP64) k_fma_probe<double><<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((double*)d_out, iters, 0.999999, 1e-6);
+    else if (prec == HEGET_FP32) k_fma_probe<float><<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((float*)d_out, iters, 0.9999f, 1e-4f);
+    else return fail(HEGET_EINVAL, "heget_fma_probe: unknown precision");
+    CU(cudaGetLastError());
+    *flops = 16.0 * (double)iters * (double)n_threads;
+    return HEGET_OK;
+}
 
 heget_status_t heget_process_create(const char* process, double sqrt_s_hat, double alpha_s, const heget_cuts_t* cuts,
                                     heget_precision_t prec, heget_process_t** out) {

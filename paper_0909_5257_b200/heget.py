@@ -17,7 +17,7 @@ FP64, FP32 = 0, 1
 HEL_SUM, HEL_SAMPLE, HEL_FIXED = 0, 1, 2
 
 EXPORTS = ["heget_process_create", "heget_process_info", "heget_color_matrix", "heget_sample_momenta", "heget_eval_me2",
-           "heget_run_host", "heget_set_lanes", "heget_destroy", "heget_last_error", "heget_launch_count"]
+           "heget_run_host", "heget_set_lanes", "heget_fma_probe", "heget_destroy", "heget_last_error", "heget_launch_count"]
 
 
 class HegetError(RuntimeError):
@@ -58,6 +58,7 @@ def lib():
         L.heget_eval_me2.argtypes = [vp, vp, u64, C.c_int, vp, u64, u64, vp, vp]
         L.heget_run_host.argtypes = [vp, u64, u64, u64, vp, vp, vp, C.c_int, vp, vp, vp]
         L.heget_set_lanes.argtypes = [vp, C.c_int]
+        L.heget_fma_probe.argtypes = [C.c_int, u64, vp, u64, C.POINTER(C.c_double), vp]
         L.heget_destroy.argtypes = [vp]
         L.heget_destroy.restype = None
         _lib = L
@@ -169,6 +170,15 @@ class Process:
                                     _hptr(mom_out, torch.float64, nm, "mom_out"), _hptr(weight, torch.float64, n_events, "weight"),
                                     mode, helbuf, _hptr(out, self.dtype, n_events, "out"), _stream(stream)))
         return out
+
+
+def fma_probe(precision, iters, n_threads, stream=None):
+    """heget_fma_probe: enqueue the FMA-chain microbenchmark; returns the flops it performs."""
+    dt = torch.float64 if precision == FP64 else torch.float32
+    out = torch.empty(n_threads, dtype=dt, device="cuda")
+    fl = C.c_double()
+    _check(lib().heget_fma_probe(precision, iters, C.c_void_p(out.data_ptr()), n_threads, C.byref(fl), _stream(stream)))
+    return fl.value
 
 
 def shard_range(n_events, rank, world_size):
