@@ -29,6 +29,7 @@ CASES = [
     ("u u > u u g g", 1000.0, 2, 4099),
     ("u u~ > g g g g", 1500.0, 9, 1027),
     ("g g > g g g g", 1500.0, 3, 4096),
+    ("u u~ > g g g g g", 2000.0, 4, 2048),
 ]
 
 
