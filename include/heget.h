@@ -66,9 +66,10 @@ typedef struct {
     double sym_factor;         /* 1/prod k!                                         */
     double flops_per_event;    /* counted by the generator from the code it emitted, HEL_SUM, FMA = 2             */
     double flops_per_helicity;
-    int regs_per_thread;       /* of the kernel HEL_SUM launches at large n_events, this precision                */
+    int regs_per_thread;       /* of the kernel variant heget_set_lanes currently selects, this precision         */
     int local_bytes_per_thread;/* stack frame (spills) of the same kernel; 0 = everything stays in registers      */
     int threads_per_block;
+    int lanes_wide;            /* helicity lanes per event of the wide kernel variant (see heget_set_lanes)        */
 } heget_info_t;
 
 /* Build (or look up) the specialised kernels of one process.
@@ -120,8 +121,10 @@ heget_status_t heget_run_host(heget_process_t* proc, uint64_t seed, uint64_t fir
                               const double* h_mom_in, double* h_mom_out, double* h_weight, heget_hel_mode_t mode,
                               const int8_t* hel, void* h_me2, void* cuda_stream);
 
-/* Choose the number of helicity lanes per event for HEL_SUM (a power of two the kernel was built with, or 0 = automatic:
- * several lanes per event for small batches, one event per thread for large ones). */
+/* Choose the kernel variant: `lanes` threads share one event and split its helicity configurations among them.
+ * 0 = automatic (the wide variant: info.lanes_wide = the largest power of two <= 32 dividing n_hel_eval, so a warp works
+ * on 32/lanes events, event-cache reads are broadcasts and the per-event prologue is spread over the lanes);
+ * 1 = one event per thread (not built for processes with >= 6 legs); lanes_wide = the wide variant. Else HEGET_EINVAL. */
 heget_status_t heget_set_lanes(heget_process_t* proc, int lanes);
 
 void heget_destroy(heget_process_t* proc);          /* NULL is allowed */

@@ -94,7 +94,7 @@ def build_library(force=False):
 
 def _compile_plugin(cu, so, prec, nlegs):
     cmd = [NVCC, "-std=c++17", "-O3"] + ARCH + ["-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v",
-           "-DHG_ONLY_PREC=%d" % prec] + (["-DHG_NO_LANES8"] if nlegs >= 6 else []) + \
+           "-DHG_ONLY_PREC=%d" % prec] + (["-DHG_NO_LANES1"] if nlegs >= 6 else []) + \
           ["-I" + os.path.join(CSRC, "device"), "-o", so + ".tmp", cu]
     dt = _run(cmd, log=so[:-3] + ".log")
     os.replace(so + ".tmp", so)

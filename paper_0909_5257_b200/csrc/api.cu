@@ -96,7 +96,7 @@ heget_status_t load_plugin(const std::string& name, const std::string& tag, int 
     if (rc != 0) return fail(HEGET_ECOMPILE, "generator failed for '%s': %s", name.c_str(), msg);
     const char* nvcc = getenv("HEGET_NVCC");
     const std::string cmd = std::string(nvcc ? nvcc : "nvcc") + " -std=c++17 -O3 -gencode arch=compute_100a,code=sm_100a -lineinfo -shared -Xcompiler -fPIC" +
-                            " -DHG_ONLY_PREC=" + (prec == 0 ? "0" : "1") + (n_legs >= 6 ? " -DHG_NO_LANES8" : "") + " -I'" + lib_dir() + "/csrc/device' -o '" + tmp +
+                            " -DHG_ONLY_PREC=" + (prec == 0 ? "0" : "1") + (n_legs >= 6 ? " -DHG_NO_LANES1" : "") + " -I'" + lib_dir() + "/csrc/device' -o '" + tmp +
                             "' '" + cu + "' > '" + log + "' 2>&1";
     if (system(cmd.c_str()) != 0) return fail(HEGET_ECOMPILE, "nvcc failed for '%s' (see %s)", name.c_str(), log.c_str());
     if (rename(tmp.c_str(), dst.c_str()) != 0) return fail(HEGET_ECOMPILE, "cannot install %s", dst.c_str());
@@ -182,7 +182,10 @@ void heget_destroy(heget_process_t* p) {
 
 heget_status_t heget_set_lanes(heget_process_t* p, int lanes) {
     if (!p) return fail(HEGET_EINVAL, "heget_set_lanes: NULL handle");
-    if (lanes != 0 && lanes != 1 && lanes != 8) return fail(HEGET_EINVAL, "heget_set_lanes: lanes must be 0, 1 or 8");
+    const hg::ProcDesc* d = p->d;
+    const bool ok = lanes == 0 || (lanes == 1 && (d->lanes_avail & 1)) || (lanes == d->lanes_wide && (d->lanes_avail & 2));
+    if (!ok) return fail(HEGET_EINVAL, "heget_set_lanes: lanes = %d is not built for '%s' (0 = automatic%s, wide = %d)", lanes, d->name,
+                         (d->lanes_avail & 1) ? ", 1" : "", d->lanes_wide);
     p->lanes = lanes; return HEGET_OK;
 }
 
@@ -194,12 +197,12 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
     o->n_color = d->n_color; o->n_color_eval = d->n_color_eval; o->n_color_reduced = d->n_color_reduced;
     o->avg_spin = d->avg_spin; o->avg_color = d->avg_color; o->sym_factor = d->sym_factor;
     o->flops_per_event = d->flops_per_event; o->flops_per_helicity = d->flops_per_hel;
-    o->threads_per_block = d->block[p->prec];
+    o->threads_per_block = d->block[p->prec]; o->lanes_wide = d->lanes_wide;
     o->regs_per_thread = -1; o->local_bytes_per_thread = -1;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {
         hg::KernelInfo ki;
-        if (d->kernel_info(p->prec, 1, &ki) == 0) { o->regs_per_thread = ki.regs; o->local_bytes_per_thread = ki.local_bytes; }
+        if (d->kernel_info(p->prec, p->lanes, &ki) == 0) { o->regs_per_thread = ki.regs; o->local_bytes_per_thread = ki.local_bytes; o->threads_per_block = ki.block; }
         else cudaGetLastError();
     } else cudaGetLastError();
     return HEGET_OK;

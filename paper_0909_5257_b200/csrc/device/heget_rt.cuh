@@ -25,7 +25,7 @@ struct LaunchArgs {
     cudaStream_t stream;
 };
 
-struct KernelInfo { int regs, local_bytes, smem_static, max_threads; };
+struct KernelInfo { int regs, local_bytes, smem_static, max_threads, block; };
 
 struct ProcDesc {
     const char* name;           // canonical process string, e.g. "g g > g g g"
@@ -48,7 +48,9 @@ struct ProcDesc {
     const signed char* hel_table;       // [n_hel_eval][n_ext] physical helicities of the kernel's enumeration
     int (*launch)(int prec, const LaunchArgs&);                 // returns cudaError_t
     int (*kernel_info)(int prec, int lanes, KernelInfo*);       // registers / local memory of the compiled kernel
-    int block[2];               // threads per block, FP64 / FP32
+    int block[2];               // threads per block of the default (widest) variant, FP64 / FP32
+    int lanes_wide;             // helicity lanes per event of the wide variant (power of two <= 32 dividing n_hel_eval)
+    int lanes_avail;            // bit 0: the one-event-per-thread variant is compiled in, bit 1: the wide variant is
     ProcDesc* next;
 };
 
@@ -61,25 +63,47 @@ struct ProcDesc {
 #endif
 #if defined(__CUDACC__) || defined(HG_HOST_DEBUG)
 // ---- device helpers used by the generated code ------------------------------------------------------------------------
+// Reads of the per-event cache are helicity-loop invariant: left to itself the compiler hoists all of them out of the
+// helicity loop and holds ~100 values in registers for the whole body, which is what spills.  A volatile read stays where
+// the schedule put it (one LDS per use, next to the vertex call that consumes it).  Measured on C2 (profiles/): FP64
+// 12.6 -> 26 TFLOP/s with volatile reads (stack frame 2200 -> 730 B); FP32, whose registers hold twice as many values and
+// whose FMA rate is twice as far ahead of the shared-memory pipe, is faster with the hoisted copy (56 vs 48 TFLOP/s).
+template <typename T> __device__ __forceinline__ T ldc(const T* p) {
+#if defined(HG_CACHE_VOLATILE32)
+    constexpr bool vol = true;
+#elif defined(HG_CACHE_HOISTABLE64)
+    constexpr bool vol = false;
+#else
+    constexpr bool vol = sizeof(T) == 8;
+#endif
+    if constexpr (vol) return *reinterpret_cast<const volatile T*>(p); else return *p;
+}
+// Between two operations of the generated schedule: keeps the compiler from hoisting the next operation's cache reads (and
+// with them its arithmetic) far ahead, which is what stretches live ranges beyond the schedule's own small live set.
+#if defined(HG_NO_FENCE) || !defined(__CUDA_ARCH__)
+#define HG_FENCE do {} while (0)
+#else
+#define HG_FENCE asm volatile("" ::: "memory")
+#endif
 template <typename T> __device__ __forceinline__ mom4<T> ldk(const T* ev, int slot, int stride) {
     mom4<T> k;
-    k.p[0] = ev[(slot + 0) * stride]; k.p[1] = ev[(slot + 1) * stride]; k.p[2] = ev[(slot + 2) * stride]; k.p[3] = ev[(slot + 3) * stride];
+    k.p[0] = ldc(ev + (slot + 0) * stride); k.p[1] = ldc(ev + (slot + 1) * stride); k.p[2] = ldc(ev + (slot + 2) * stride); k.p[3] = ldc(ev + (slot + 3) * stride);
     return k;
 }
 template <typename T> __device__ __forceinline__ vec4<T> ldv(const T* ev, int slot, int stride, T lambda) {   // vxxxxx, helicity part
     vec4<T> w;
     w.v[0] = mk<T>(T(0), T(0));
-    w.v[1] = mk<T>(lambda * ev[(slot + 0) * stride], ev[(slot + 3) * stride]);
-    w.v[2] = mk<T>(lambda * ev[(slot + 1) * stride], ev[(slot + 4) * stride]);
-    w.v[3] = mk<T>(lambda * ev[(slot + 2) * stride], ev[(slot + 5) * stride]);
+    w.v[1] = mk<T>(lambda * ldc(ev + (slot + 0) * stride), ldc(ev + (slot + 3) * stride));
+    w.v[2] = mk<T>(lambda * ldc(ev + (slot + 1) * stride), ldc(ev + (slot + 4) * stride));
+    w.v[3] = mk<T>(lambda * ldc(ev + (slot + 2) * stride), ldc(ev + (slot + 5) * stride));
     return w;
 }
 template <typename T> __device__ __forceinline__ sp2<T> ldi(const T* ev, int slot, int stride, T chi) {       // ixxxxx, helicity part
-    const T s[3] = {ev[slot * stride], ev[(slot + 1) * stride], ev[(slot + 2) * stride]};
+    const T s[3] = {ldc(ev + slot * stride), ldc(ev + (slot + 1) * stride), ldc(ev + (slot + 2) * stride)};
     return ixxxxx<T>(s, chi);
 }
 template <typename T> __device__ __forceinline__ sp2<T> ldo(const T* ev, int slot, int stride, T chi) {       // oxxxxx, helicity part
-    const T s[3] = {ev[slot * stride], ev[(slot + 1) * stride], ev[(slot + 2) * stride]};
+    const T s[3] = {ldc(ev + slot * stride), ldc(ev + (slot + 1) * stride), ldc(ev + (slot + 2) * stride)};
     return oxxxxx<T>(s, chi);
 }
 

@@ -134,27 +134,68 @@ struct Emitter {
         done[c] = 1;
         if (C.kind != CK_LEAF) { Op o; o.closing = false; o.id = c; ops.push_back(o); }
     }
+    // transitive set of not-yet-computed currents under c (post-order), without marking them done
+    void missing(int c, const std::vector<char>& done, std::vector<int>& stamp, int mark, std::vector<int>& out) const {
+        if (done[c] || stamp[c] == mark) return;
+        stamp[c] = mark;
+        const Cur& C = G.cur[c];
+        if (C.kind == CK_LEAF) return;
+        for (int j = 0; j < 3; ++j) if (C.ch[j] >= 0) missing(C.ch[j], done, stamp, mark, out);
+        out.push_back(c);
+    }
     void schedule() {
         const int nc = (int)G.cur.size(), nl = (int)G.closings.size();
-        std::vector<char> done(nc, 0), cdone(nl, 0);
+        std::vector<char> done(nc, 0);
         std::vector<int> stamp(nc, -1);
         int mark = 0;
-        // closings are taken in the order that needs the fewest not-yet-computed currents (ties: generator order);
-        // to stay O(n log n) for the big processes the scan window is bounded
+        // uses[c] = ops (currents that will certainly be needed, closings) still to read current c
+        std::vector<char> needed(nc, 0);
+        { std::vector<int> st; for (int l = 0; l < nl; ++l) for (int j = 0; j < 4; ++j) if (G.closings[l].c[j] >= 0) st.push_back(G.closings[l].c[j]);
+          while (!st.empty()) { int c = st.back(); st.pop_back(); if (needed[c]) continue; needed[c] = 1; for (int j = 0; j < 3; ++j) if (G.cur[c].ch[j] >= 0) st.push_back(G.cur[c].ch[j]); } }
+        std::vector<int> uses(nc, 0);
+        for (int c = 0; c < nc; ++c) if (needed[c]) for (int j = 0; j < 3; ++j) if (G.cur[c].ch[j] >= 0) uses[G.cur[c].ch[j]]++;
+        for (int l = 0; l < nl; ++l) for (int j = 0; j < 4; ++j) if (G.closings[l].c[j] >= 0) uses[G.closings[l].c[j]]++;
+        // Greedy for a small peak of simultaneously live currents (each is 8 or 16 registers): take the closing whose
+        // execution changes the number of live currents the least (new currents that stay alive minus currents that die),
+        // then the one that needs the fewest new currents, then generator order.
         std::vector<int> pending; for (int l = 0; l < nl; ++l) pending.push_back(l);
+        std::vector<int> tmp(nc, 0), miss;
         while (!pending.empty()) {
-            int best = -1, bestc = 1 << 30; size_t bestpos = 0;
+            int best = -1; long bestscore = 1L << 40; size_t bestpos = 0;
             for (size_t k = 0; k < pending.size(); ++k) {
                 const Closing& cl = G.closings[pending[k]];
-                int c = 0; ++mark;
-                for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) c += cost_missing(cl.c[j], done, stamp, mark);
-                if (c < bestc) { bestc = c; best = pending[k]; bestpos = k; if (c == 0) break; }
+                ++mark; miss.clear();
+                for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) missing(cl.c[j], done, stamp, mark, miss);
+                // simulate the use counts
+                std::vector<int> touched;
+                for (size_t m = 0; m < miss.size(); ++m) for (int j = 0; j < 3; ++j) { const int ch = G.cur[miss[m]].ch[j]; if (ch >= 0) { if (!tmp[ch]) touched.push_back(ch); tmp[ch]++; } }
+                for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) { const int ch = cl.c[j]; if (!tmp[ch]) touched.push_back(ch); tmp[ch]++; }
+                int born = 0, dying = 0, closest = 255;
+                for (size_t m = 0; m < miss.size(); ++m) if (uses[miss[m]] - tmp[miss[m]] > 0) ++born;          // new and still needed afterwards
+                for (size_t q = 0; q < touched.size(); ++q) {
+                    const int ch = touched[q];
+                    if (G.cur[ch].kind == CK_LEAF || !done[ch]) continue;
+                    const int left = uses[ch] - tmp[ch];
+                    if (left == 0) ++dying;
+                    // "finish what was started": among equal changes prefer the closing that brings a big live current nearest to its death
+                    const int key = left * 4 - G.cur[ch].size; if (key < closest) closest = key < 0 ? 0 : key;
+                }
+                for (size_t q = 0; q < touched.size(); ++q) tmp[touched[q]] = 0;
+                const long score = (long)(born - dying) * (1L << 20) + (long)closest * 256 + (long)miss.size();
+                if (score < bestscore) { bestscore = score; best = pending[k]; bestpos = k; }
             }
             const Closing& cl = G.closings[best];
-            for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) need(cl.c[j], done);
+            ++mark; miss.clear();
+            for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) missing(cl.c[j], done, stamp, mark, miss);
+            for (size_t m = 0; m < miss.size(); ++m) {
+                done[miss[m]] = 1; Op o; o.closing = false; o.id = miss[m]; ops.push_back(o);
+                for (int j = 0; j < 3; ++j) if (G.cur[miss[m]].ch[j] >= 0) uses[G.cur[miss[m]].ch[j]]--;
+            }
+            for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) uses[cl.c[j]]--;
             Op o; o.closing = true; o.id = best; ops.push_back(o);
             pending.erase(pending.begin() + bestpos);
         }
+        const int ncd = nc; (void)ncd;
         // liveness
         last_use.assign(nc, -1);
         for (size_t k = 0; k < ops.size(); ++k) {

@@ -81,7 +81,8 @@ def test_handle_calls_without_device(lib):
     assert lib.heget_eval_me2(P._h, None, 8, 9, None, 0, 0, None, None) == hg.EINVAL
     assert lib.heget_eval_me2(P._h, None, 8, hg.HEL_FIXED, None, 0, 0, None, None) == hg.EINVAL
     assert lib.heget_set_lanes(P._h, 3) == hg.EINVAL
-    assert lib.heget_set_lanes(P._h, 8) == hg.OK
+    assert P.info.lanes_wide == 8            # 8 non-vanishing helicity configurations
+    assert lib.heget_set_lanes(P._h, 8) == hg.OK and lib.heget_set_lanes(P._h, 1) == hg.OK and lib.heget_set_lanes(P._h, 0) == hg.OK
     P.close()
     P.close()
 

@@ -104,8 +104,12 @@ def test_me2_fp64_matches_oracle(events, oracle_process, name, sqrt_s, seed, n):
     P = hg.Process(name, sqrt_s, precision="fp64")
     ref = oracle_process(name).me2(mom_h)
     assert np.all(ref > 0)
-    for lanes in (1, 8):
-        P.set_lanes(lanes)
+    for lanes in sorted({1, P.info.lanes_wide}):
+        try:
+            P.set_lanes(lanes)
+        except hg.HegetError as e:        # the one-event-per-thread variant is not built for the big processes
+            assert e.status == hg.EINVAL and lanes == 1 and P.n_ext >= 6
+            continue
         out = P.eval_me2(mom).cpu().numpy()
         err = rel_err(out, ref)
         k = int(err.argmax())
