@@ -142,6 +142,8 @@ def run_ours(a):
 
     name, sqrt_s, E, seed = CONFIGS[a.config]
     P = hg.Process(name, sqrt_s, precision=a.precision)
+    if a.lanes:
+        P.set_lanes(a.lanes)
     info = P.info
     ne = info.n_ext
     first = rank * E                      # weak scaling: rank r evaluates global events [rE, (r+1)E)
@@ -250,7 +252,7 @@ def run_ours(a):
                                % (a.config, name, sqrt_s, E, seed, info.n_hel),
                    "precision": a.precision, "l2": "flushed between steps" if need_flush else "inputs larger than L2 (%d MiB momenta)" % (mom.numel() * 8 >> 20),
                    "parallelism": "events sharded over %d GPU(s), no collective" % world},
-        "roofline": {"bound": "alu", "kernel": "heget_eval_me2 (%d-thread blocks, %d regs, %d B local)" % (info.threads_per_block, info.regs_per_thread, info.local_bytes_per_thread),
+        "roofline": {"bound": "alu", "kernel": "heget_eval_me2 (%d lanes/event, %d-thread blocks, %d regs, %d B local)" % (info.lanes, info.threads_per_block, info.regs_per_thread, info.local_bytes_per_thread),
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
                      "peak_kind": "nominal %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md)" % (SM_COUNT, lanes, sm_max),
                      "fma_probe_tflops": probe, "frac_of_probe": achieved / probe,
@@ -275,6 +277,7 @@ def main():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lanes", type=int, default=0, help="kernel variant (heget_set_lanes); 0 = automatic")
     a = ap.parse_args()
     a.warmup = max(a.warmup, 3) if a.impl == "ours" else a.warmup
     if a.impl == "reference":

@@ -70,6 +70,7 @@ typedef struct {
     int local_bytes_per_thread;/* stack frame (spills) of the same kernel; 0 = everything stays in registers      */
     int threads_per_block;
     int lanes_wide;            /* helicity lanes per event of the wide kernel variant (see heget_set_lanes)        */
+    int lanes;                 /* lanes per event of the variant currently selected                               */
 } heget_info_t;
 
 /* Build (or look up) the specialised kernels of one process.
@@ -122,7 +123,7 @@ heget_status_t heget_run_host(heget_process_t* proc, uint64_t seed, uint64_t fir
                               const int8_t* hel, void* h_me2, void* cuda_stream);
 
 /* Choose the kernel variant: `lanes` threads share one event and split its helicity configurations among them.
- * 0 = automatic (the wide variant: info.lanes_wide = the largest power of two <= 32 dividing n_hel_eval, so a warp works
+ * 0 = automatic (FP64: the wide variant, FP32: one event per thread where built, else wide; wide = info.lanes_wide = the largest power of two <= 32 dividing n_hel_eval, so a warp works
  * on 32/lanes events, event-cache reads are broadcasts and the per-event prologue is spread over the lanes);
  * 1 = one event per thread (not built for processes with >= 6 legs); lanes_wide = the wide variant. Else HEGET_EINVAL. */
 heget_status_t heget_set_lanes(heget_process_t* proc, int lanes);

@@ -80,11 +80,24 @@ template <typename T> __device__ __forceinline__ T ldc(const T* p) {
 }
 // Between two operations of the generated schedule: keeps the compiler from hoisting the next operation's cache reads (and
 // with them its arithmetic) far ahead, which is what stretches live ranges beyond the schedule's own small live set.
-#if defined(HG_NO_FENCE) || !defined(__CUDA_ARCH__)
-#define HG_FENCE do {} while (0)
+template <typename T> __device__ __forceinline__ void fence() {
+#if defined(__CUDA_ARCH__) && !defined(HG_NO_FENCE)
+#if defined(HG_NO_FENCE32)
+    if constexpr (sizeof(T) == 8) asm volatile("" ::: "memory");
 #else
-#define HG_FENCE asm volatile("" ::: "memory")
+    asm volatile("" ::: "memory");
 #endif
+#endif
+}
+template <typename T> __host__ __device__ constexpr bool leaf_reload() {
+#if defined(HG_LEAF_RELOAD32)
+    return true;
+#elif defined(HG_LEAF_HOLD64)
+    return false;
+#else
+    return sizeof(T) == 8;
+#endif
+}
 template <typename T> __device__ __forceinline__ mom4<T> ldk(const T* ev, int slot, int stride) {
     mom4<T> k;
     k.p[0] = ldc(ev + (slot + 0) * stride); k.p[1] = ldc(ev + (slot + 1) * stride); k.p[2] = ldc(ev + (slot + 2) * stride); k.p[3] = ldc(ev + (slot + 3) * stride);

@@ -35,7 +35,7 @@ class Info(C.Structure):
                 ("n_topologies", C.c_int), ("n_color", C.c_int), ("n_color_eval", C.c_int), ("n_color_reduced", C.c_int),
                 ("avg_spin", C.c_double), ("avg_color", C.c_double), ("sym_factor", C.c_double),
                 ("flops_per_event", C.c_double), ("flops_per_helicity", C.c_double),
-                ("regs_per_thread", C.c_int), ("local_bytes_per_thread", C.c_int), ("threads_per_block", C.c_int), ("lanes_wide", C.c_int)]
+                ("regs_per_thread", C.c_int), ("local_bytes_per_thread", C.c_int), ("threads_per_block", C.c_int), ("lanes_wide", C.c_int), ("lanes", C.c_int)]
 
 
 _lib = None
