@@ -29,6 +29,9 @@ CONFIGS = {   # BASELINE.json configs / SURVEY.md 8 table: process, sqrt(s_hat) 
 }
 ORACLE_SAMPLE = {"C1": 1 << 14, "C2": 1 << 15, "C3": 1 << 13, "C4": 1 << 10, "C5": 1 << 7}   # ~10-30 s of host work
 METRIC = "helicity-summed |M|^2 events/sec per process on 1 B200; % of FP64/FP32 peak"
+# dram__bytes_read.sum + dram__bytes_write.sum of the |M|^2 kernel, bytes per launch, from the committed `ncu --set full` captures
+TRAFFIC = {("C2", "fp64"): 178.3e6, ("C2", "fp32"): 175.0e6}
+TRAFFIC_NOTE = {("C2", "fp64"): "profiles/r1b_ncu_c2.md (algorithmic: 168 MB in + 8 MB out)", ("C2", "fp32"): "profiles/r1b_ncu_c2.md (algorithmic: 168 MB in + 4 MB out)"}
 SM_COUNT, FP64_LANES, FP32_LANES = 148, 64, 128      # per SM; DESIGN.md "Roofline" derives the ALU peak from these
 
 
@@ -141,6 +144,8 @@ def run_ours(a):
         return float(t.item())
 
     name, sqrt_s, E, seed = CONFIGS[a.config]
+    if a.events:
+        E = a.events                      # profiling aid only: not BASELINE.json's size, the workload string says so
     P = hg.Process(name, sqrt_s, precision=a.precision)
     if a.lanes:
         P.set_lanes(a.lanes)
@@ -252,8 +257,8 @@ def run_ours(a):
                                % (a.config, name, sqrt_s, E, seed, info.n_hel),
                    "precision": a.precision, "l2": "flushed between steps" if need_flush else "inputs larger than L2 (%d MiB momenta)" % (mom.numel() * 8 >> 20),
                    "parallelism": "events sharded over %d GPU(s), no collective" % world},
-        "roofline": {"bound": "alu", "kernel": "heget_eval_me2 (%d lanes/event, %d-thread blocks, %d regs, %d B local)" % (info.lanes, info.threads_per_block, info.regs_per_thread, info.local_bytes_per_thread),
-                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+        "roofline": {"bound": "alu", "traffic_note": TRAFFIC_NOTE.get((a.config, a.precision)) if not a.events else None, "kernel": "heget_eval_me2 (%d lanes/event, %d-thread blocks, %d regs, %d B local)" % (info.lanes, info.threads_per_block, info.regs_per_thread, info.local_bytes_per_thread),
+                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": TRAFFIC.get((a.config, a.precision)) if not a.events else None,
                      "peak_kind": "nominal %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md)" % (SM_COUNT, lanes, sm_max),
                      "fma_probe_tflops": probe, "frac_of_probe": achieved / probe,
                      "flops_per_event": info.flops_per_event, "kernel_ms": k_ms, "sampling_kernel_ms": s_ms,
@@ -278,6 +283,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, help="kernel variant (heget_set_lanes); 0 = automatic")
+    ap.add_argument("--events", type=int, default=0, help="override the events per step (ncu captures of the big configs)")
     a = ap.parse_args()
     a.warmup = max(a.warmup, 3) if a.impl == "ours" else a.warmup
     if a.impl == "reference":

@@ -229,3 +229,30 @@ def test_no_spill_report_and_launch_counter():
     mom = P.sample_momenta(0, 256)
     P.eval_me2(mom)
     assert hg.launch_count() == c0 + 2
+
+
+@pytest.mark.parametrize("cfg,precision", [("C2", "fp64"), ("C2", "fp32"), ("C3", "fp64")])
+def test_full_size_bench_configuration(oracle_process, cfg, precision):
+    """BASELINE.json's full size in the launch configuration bench.py times (automatic lanes): sampled events against the
+    oracle one by one, plus what holds at any size -- every |M|^2 positive and finite, and Bose symmetry: exchanging the momenta
+    of two identical final-state gluons leaves |M|^2 unchanged (SURVEY.md 8(c) 'permutation symmetry')."""
+    from bench import CONFIGS
+    name, sqrt_s, E, seed = CONFIGS[cfg]
+    P = hg.Process(name, sqrt_s, precision=precision)
+    mom = P.sample_momenta(seed, E)
+    out = P.eval_me2(mom)
+    assert bool(torch.isfinite(out).all()) and float(out.min()) > 0.0
+    idx = torch.randperm(E, generator=torch.Generator().manual_seed(7))[:256].sort().values
+    ref = oracle_process(name).me2(mom[:, :, idx.cuda()].cpu().numpy())
+    err = rel_err(out[idx.cuda()].cpu().numpy().astype(np.float64), ref)
+    if precision == "fp64":
+        assert err.max() <= TOL64
+    else:
+        assert np.median(err) <= TOL32_MEDIAN and err.max() <= TOL32_MAX
+    gl = [i for i, t in enumerate(name.split(">")[1].split()) if t == "g"]
+    a, b = 2 + gl[-2], 2 + gl[-1]                       # the last two final-state gluons
+    swapped = mom.clone()
+    swapped[a], swapped[b] = mom[b], mom[a]
+    out2 = P.eval_me2(swapped)
+    sym = ((out2 - out).abs() / out).max().item()
+    assert sym <= (1e-11 if precision == "fp64" else 1e-3)
