@@ -31,6 +31,20 @@
 #define HG_HD inline
 #endif
 
+// vertex-level functions: inlined into the generated body by default; -DHG_CALL_VERTEX makes them real calls so that a long
+// body holds one copy of each (an experiment against the instruction-fetch bound of the big processes)
+#if defined(HG_CALL_VERTEX) && defined(__CUDACC__)
+#define HG_VX __device__ __noinline__
+#define HG_CV4 const vec4<T>
+#define HG_CM4 const mom4<T>
+#define HG_CS2 const sp2<T>
+#else
+#define HG_VX HG_HD
+#define HG_CV4 const vec4<T>&
+#define HG_CM4 const mom4<T>&
+#define HG_CS2 const sp2<T>&
+#endif
+
 namespace hg {
 
 template <typename T> struct cx { T re, im; };
@@ -130,8 +144,8 @@ template <typename T> HG_HD sp2<T> oxxxxx(const T* s, T chi) {
 
 // vvvxxx: amplitude of the ggg vertex from three (on- or off-shell) gluon wavefunctions; colour factor i f^{abc}
 // (eq. 27).  Arguments as eq. 24 plus the momenta flowing INTO the vertex.
-template <typename T> HG_HD cx<T> vvvxxx(const vec4<T>& ga, const mom4<T>& ka, const vec4<T>& gb, const mom4<T>& kb,
-                                         const vec4<T>& gc, const mom4<T>& kc, T g) {
+template <typename T> HG_VX cx<T> vvvxxx(HG_CV4 ga, HG_CM4 ka, HG_CV4 gb, HG_CM4 kb,
+                                         HG_CV4 gc, HG_CM4 kc, T g) {
     const cx<T> ab = vdot(ga, gb), bc = vdot(gb, gc), ca = vdot(gc, ga);
     const cx<T> v = ab * kdot(ka - kb, gc) + bc * kdot(kb - kc, ga) + ca * kdot(kc - ka, gb);
     return g * v;
@@ -141,7 +155,7 @@ template <typename T> HG_HD cx<T> vvvxxx(const vec4<T>& ga, const mom4<T>& ka, c
 // PAPER.md:292-313; surviving fragments of List 2); colour factor i f^{abc} (eq. 30).
 // q = -(ka + kb) is the momentum of the third leg flowing into the vertex; inv_q2 = 1/q^2.
 //   j^mu = g/q^2 [ (a.b)(ka-kb)^mu + b^mu ((kb-q).a) + a^mu ((q-ka).b) ],  kb - q = ka + 2 kb,  q - ka = -(2 ka + kb)
-template <typename T> HG_HD vec4<T> jvvxx0(const vec4<T>& ga, const mom4<T>& ka, const vec4<T>& gb, const mom4<T>& kb, T g, T inv_q2) {
+template <typename T> HG_VX vec4<T> jvvxx0(HG_CV4 ga, HG_CM4 ka, HG_CV4 gb, HG_CM4 kb, T g, T inv_q2) {
     const T gs = g * inv_q2;
     const cx<T> ab = gs * vdot(ga, gb);
     const cx<T> sa = gs * kdot(ka + kb + kb, ga);
@@ -192,12 +206,12 @@ template <typename T> HG_HD void jgggx03(const vec4<T>& ga, const vec4<T>& gb, c
 }
 
 // piece-indexed forms used by the generated code: piece 0, 1, 2 = the argument permutations of eqs. 35a-c
-template <typename T> HG_HD cx<T> ggggxxp(const vec4<T>& ga, const vec4<T>& gb, const vec4<T>& gc, const vec4<T>& gd, int piece) {
+template <typename T> HG_VX cx<T> ggggxxp(HG_CV4 ga, HG_CV4 gb, HG_CV4 gc, HG_CV4 gd, int piece) {
     if (piece == 0) return ggggxx<T>(ga, gb, gc, gd, T(1));
     if (piece == 1) return ggggxx<T>(ga, gc, gd, gb, T(1));
     return ggggxx<T>(ga, gd, gb, gc, T(1));
 }
-template <typename T> HG_HD vec4<T> jgggx0p(const vec4<T>& ga, const vec4<T>& gb, const vec4<T>& gc, int piece, T inv_q2) {
+template <typename T> HG_VX vec4<T> jgggx0p(HG_CV4 ga, HG_CV4 gb, HG_CV4 gc, int piece, T inv_q2) {
     if (piece == 0) return jgggx0<T>(ga, gb, gc, T(1), inv_q2);      // (b.c) a - (a.c) b
     if (piece == 1) return jgggx0<T>(gc, ga, gb, T(1), inv_q2);      // (a.b) c - (c.b) a
     return jgggx0<T>(gb, gc, ga, T(1), inv_q2);                      // (c.a) b - (b.a) c
@@ -236,25 +250,25 @@ template <typename T> HG_HD sp2<T> kmul_row(const sp2<T>& f, const mom4<T>& k, T
 }
 
 // iovxx0: amplitude of the qqg vertex (eq. 20; g[0] = g[1] = g, eq. 21):  g fo S(vc; chi) fi
-template <typename T> HG_HD cx<T> iovxx0(const sp2<T>& fi, const sp2<T>& fo, const vec4<T>& vc, T chi, T g) {
+template <typename T> HG_VX cx<T> iovxx0(HG_CS2 fi, HG_CS2 fo, HG_CV4 vc, T chi, T g) {
     const sp2<T> t = smul_col(vc, chi, fi);
     return g * (fo.s[0] * t.s[0] + fo.s[1] * t.s[1]);
 }
 // fvixx0: off-shell flowing-in quark from a flowing-in quark and a gluon, massless propagator.
 // k = momentum of the new line along the fermion arrow (= sum of the incoming momenta behind it); inv_k2 = 1/k^2.
 //   fvi = -g/k^2  S(k; -chi) S(vc; chi) fi
-template <typename T> HG_HD sp2<T> fvixx0(const sp2<T>& fi, const vec4<T>& vc, const mom4<T>& k, T chi, T g, T inv_k2) {
+template <typename T> HG_VX sp2<T> fvixx0(HG_CS2 fi, HG_CV4 vc, HG_CM4 k, T chi, T g, T inv_k2) {
     return kmul_col(k, -chi, smul_col(vc, chi, fi), -g * inv_k2);
 }
 // fvoxx0: off-shell flowing-out quark from a flowing-out quark and a gluon.  Here the arrow points from the root towards
 // the leaves, so the momentum along it is MINUS the sum of the incoming momenta behind the line: pass that sum as ksum.
 //   fvo = -g/k^2  fo S(vc; chi) S(-ksum; -chi)
-template <typename T> HG_HD sp2<T> fvoxx0(const sp2<T>& fo, const vec4<T>& vc, const mom4<T>& ksum, T chi, T g, T inv_k2) {
+template <typename T> HG_VX sp2<T> fvoxx0(HG_CS2 fo, HG_CV4 vc, HG_CM4 ksum, T chi, T g, T inv_k2) {
     return kmul_row(smul_row(fo, vc, chi), ksum, -chi, g * inv_k2);
 }
 // jioxx0: off-shell gluon from a quark pair, Feynman-gauge propagator:  j^mu = g/q^2 fo sigma_chi^mu fi,
 // sigma_chi^mu = (1, -chi sigma^i)
-template <typename T> HG_HD vec4<T> jioxx0(const sp2<T>& fi, const sp2<T>& fo, T chi, T g, T inv_q2) {
+template <typename T> HG_VX vec4<T> jioxx0(HG_CS2 fi, HG_CS2 fo, T chi, T g, T inv_q2) {
     const T c = g * inv_q2, cs = -chi * c;
     const cx<T> a00 = fo.s[0] * fi.s[0], a11 = fo.s[1] * fi.s[1], a01 = fo.s[0] * fi.s[1], a10 = fo.s[1] * fi.s[0];
     vec4<T> j;
