@@ -217,6 +217,16 @@ def run_ours(a):
     torch.cuda.synchronize()
     probe = fl / (pev[0].elapsed_time(pev[1]) * 1e-3) / 1e12
 
+    # ---- what the paper itself timed: ONE Philox-drawn helicity configuration per event, for context ------
+    P.eval_me2(mom, mode=hg.HEL_SAMPLE, seed=seed, first_event=first, out=me2)
+    hev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    hev[0].record()
+    for k in range(a.steps):
+        P.eval_me2(mom, mode=hg.HEL_SAMPLE, seed=seed + k, first_event=first, out=me2)
+    hev[1].record()
+    torch.cuda.synchronize()
+    hel_sample = E * a.steps / (hev[0].elapsed_time(hev[1]) * 1e-3)
+
     # ---- end to end through the C-ABI with HOST buffers ----------------------------------------------------------------
     h_mom = torch.empty(ne, 4, E, dtype=torch.float64).pin_memory()
     h_me2 = torch.empty(E, dtype=P.dtype).pin_memory()
@@ -267,6 +277,8 @@ def run_ours(a):
         "e2e": {"value": e2e, "unit": "events/s", "h2d_bytes_per_step": int(h_mom.numel() * 8), "d2h_bytes_per_step": int(h_me2.numel() * h_me2.element_size()),
                 "what": "heget_run_host: pinned host momenta -> device, heget_eval_me2, me2 -> pinned host, stream synchronised, per step"},
         "gpu_launches": int(launches), "clocks": clk,
+        "context": {"hel_sample_events_per_s": hel_sample,
+                    "note": "one sampled helicity configuration per event, kernel only -- the mode the paper timed (BASELINE.md); not the metric"},
     }
     print(json.dumps(line))
     if world > 1:

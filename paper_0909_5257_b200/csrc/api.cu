@@ -265,6 +265,9 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
     hg::LaunchArgs a;
     a.d_mom = d_mom; a.n_events = n_events; a.inv_sqrt_s = 1.0 / p->sqrt_s; a.out_scale = p->out_scale; a.d_me2 = d_me2;
     a.hel_mode = (int)mode; a.hel_fixed = -1; a.seed = seed; a.first_event = first_event; a.d_jbuf = 0; a.lanes = effective_lanes(p);
+    // one configuration per event: in the wide variant all lanes of an event would evaluate the same configuration, so take
+    // the one-event-per-thread variant where it is built (the big processes only have the wide one: L-fold redundant there)
+    if (mode != HEGET_HEL_SUM && p->lanes == 0 && (d->lanes_avail & 1)) a.lanes = 1;
     a.stream = (cudaStream_t)cuda_stream;
     if (mode == HEGET_HEL_FIXED) {
         for (int i = 0; i < d->n_ext; ++i) if (hel[i] != 1 && hel[i] != -1) return fail(HEGET_EINVAL, "heget_eval_me2: hel[%d] = %d is not +-1", i, (int)hel[i]);

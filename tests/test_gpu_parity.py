@@ -256,3 +256,25 @@ def test_full_size_bench_configuration(oracle_process, cfg, precision):
     out2 = P.eval_me2(swapped)
     sym = ((out2 - out).abs() / out).max().item()
     assert sym <= (1e-11 if precision == "fp64" else 1e-3)
+
+
+@pytest.mark.parametrize("name,sqrt_s,seed", [("g g > g g g g", 1500.0, 3), ("u u~ > g g g g", 1500.0, 9)])
+def test_helicity_modes_in_long_bodies(events, name, sqrt_s, seed):
+    """The big processes' bodies contain block barriers, so every thread must run the same helicity iterations in every mode:
+    the 2^n_ext HEL_FIXED terms add up to HEL_SUM, a vanishing configuration gives exactly 0, and a HEL_SAMPLE value is
+    2^n_ext times one of the terms."""
+    n = 70                                 # a ragged tail inside one block
+    P = hg.Process(name, sqrt_s)
+    mom = P.sample_momenta(seed, n)
+    full = P.eval_me2(mom).cpu().numpy()
+    ne = P.n_ext
+    terms = []
+    for bits in range(1 << ne):
+        hel = [1 if (bits >> i) & 1 else -1 for i in range(ne)]
+        terms.append(P.eval_me2(mom, mode=hg.HEL_FIXED, hel=hel).cpu().numpy())
+    terms = np.array(terms)
+    assert rel_err(terms.sum(axis=0), full).max() < 1e-12
+    assert (terms == 0).all(axis=1).sum() == (1 << ne) - P.info.n_hel_eval       # chirality-violating configurations
+    samp = P.eval_me2(mom, mode=hg.HEL_SAMPLE, seed=5).cpu().numpy()
+    for e in range(n):
+        assert np.min(np.abs(terms[:, e] * (1 << ne) - samp[e])) <= 1e-12 * max(samp[e], terms[:, e].max() * (1 << ne))
