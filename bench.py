@@ -158,6 +158,8 @@ def run_ours(a):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
     need_flush = mom.numel() * 8 < (160 << 20)
 
+    hg_count = [0]                        # kernels replayed from a CUDA graph (the library's own counter does not see replays)
+
     def step(k):
         P.sample_momenta(seed, E, first_event=first + k * world * E, mom=mom, weight=wgt)
         P.eval_me2(mom, out=me2)
@@ -166,8 +168,37 @@ def run_ours(a):
     for k in range(a.warmup):
         step(k)
     barrier()
+    # small batches (C1: 2^14 events, ~20 us of GPU work per kernel) are bound by the host's launch path: replay the step from
+    # a CUDA graph.  The captured step re-samples the same event range each replay (first_event is baked into the graph).
+    graph = None
+    if E < (1 << 17) and not a.no_graph:
+        try:
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                step(0)
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=side):
+                    step(0)
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            graph = g
+        except Exception as exc:       # capture not possible: plain launches
+            graph = None
+            sys.stderr.write("bench.py: CUDA graph capture failed (%s); timing plain launches\n" % exc)
+            torch.cuda.synchronize()
+    if graph is not None:
+        plain_step = step
+
+        def step(k):
+            graph.replay()
+            hg_count[0] += 2
+        for k in range(a.warmup):
+            step(k)
+        barrier()
     clocks = ClockSampler(local) if rank == 0 else None
     c0 = hg.launch_count()
+    hg_count[0] = 0
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * a.steps)]
     for k in range(a.steps):
         if need_flush:
@@ -176,7 +207,7 @@ def run_ours(a):
         step(a.warmup + k)
         ev[2 * k + 1].record()
     barrier()
-    launches = hg.launch_count() - c0
+    launches = hg.launch_count() - c0 + hg_count[0]
     ms = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(a.steps))
     ms = max_over_ranks(ms)
     clk = clocks.stop() if clocks else None
@@ -266,7 +297,8 @@ def run_ours(a):
         "config": {"workload": "%s: %s, sqrt_s_hat=%g GeV, %d events/step/GPU, Philox seed %d, cuts pT>20 |eta|<2.5 dR>0.4, full %d-helicity sum"
                                % (a.config, name, sqrt_s, E, seed, info.n_hel),
                    "precision": a.precision, "l2": "flushed between steps" if need_flush else "inputs larger than L2 (%d MiB momenta)" % (mom.numel() * 8 >> 20),
-                   "parallelism": "events sharded over %d GPU(s), no collective" % world},
+                   "parallelism": "events sharded over %d GPU(s), no collective" % world,
+                   "launch": "CUDA graph replay of the 2-kernel step" if graph is not None else "plain stream launches"},
         "roofline": {"bound": "alu", "traffic_note": TRAFFIC_NOTE.get((a.config, a.precision)) if not a.events else None, "kernel": "heget_eval_me2 (%d lanes/event, %d-thread blocks, %d regs, %d B local)" % (info.lanes, info.threads_per_block, info.regs_per_thread, info.local_bytes_per_thread),
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": TRAFFIC.get((a.config, a.precision)) if not a.events else None,
                      "peak_kind": "nominal %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md)" % (SM_COUNT, lanes, sm_max),
@@ -294,6 +326,7 @@ def main():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="do not replay small-batch steps from a CUDA graph")
     ap.add_argument("--lanes", type=int, default=0, help="kernel variant (heget_set_lanes); 0 = automatic")
     ap.add_argument("--events", type=int, default=0, help="override the events per step (ncu captures of the big configs)")
     a = ap.parse_args()
