@@ -41,7 +41,10 @@ typedef enum {
     HEGET_ECOMPILE = 5       /* no pre-built kernel for the process and run-time generation/compilation failed  */
 } heget_status_t;
 
-typedef enum { HEGET_FP64 = 0, HEGET_FP32 = 1 } heget_precision_t;
+/* HEGET_FP32X2: the FP32 arithmetic of HEGET_FP32 (same rounding, same tolerances, float output), executed two helicity
+ * configurations per thread on Blackwell's packed f32x2 instructions (FFMA2/FMUL2/FADD2): half the instructions per event.
+ * Needs at least one external gluon (the two configurations differ in its helicity), else HEGET_EUNSUPPORTED. */
+typedef enum { HEGET_FP64 = 0, HEGET_FP32 = 1, HEGET_FP32X2 = 2 } heget_precision_t;
 
 /* helicity treatment of eq. 12.  SUM: all 2^n_ext configurations (the graded mode, reading A8).
  * SAMPLE: one configuration per event drawn from Philox(seed, global event index), weighted by 2^n_ext -- what the paper
@@ -107,7 +110,7 @@ heget_status_t heget_sample_momenta(heget_process_t* proc, uint64_t seed, uint64
  *           p_a + p_b = sum p_final are accepted)
  *   mode    see heget_hel_mode_t;  hel = n_ext entries of +-1 (host pointer) for FIXED, else ignored;
  *           seed/first_event only matter for SAMPLE
- *   d_me2   double[n_events] (HEGET_FP64 handle) or float[n_events] (HEGET_FP32 handle)
+ *   d_me2   double[n_events] (HEGET_FP64 handle) or float[n_events] (HEGET_FP32 / HEGET_FP32X2 handle)
  * n_events == 0 is a no-op returning HEGET_OK. */
 heget_status_t heget_eval_me2(heget_process_t* proc, const double* d_mom, uint64_t n_events, heget_hel_mode_t mode,
                               const int8_t* hel, uint64_t seed, uint64_t first_event, void* d_me2, void* cuda_stream);

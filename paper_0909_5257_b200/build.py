@@ -5,7 +5,7 @@
 1. g++   csrc/gen/hegetgen.cpp                      -> bin/hegetgen        (process generator, step a0)
 2. nvcc  csrc/api.cu + csrc/gen/genlib.cpp          -> libheget.so         (C-ABI of include/heget.h + RAMBO kernel)
 3. for every process in PROCESSES: hegetgen -> kernels/gen_<tag>.cu, then one nvcc per precision
-                                                   -> kernels/heget_<tag>_f64.so, kernels/heget_<tag>_f32.so
+                                                   -> kernels/heget_<tag>_f64.so, _f32.so, _f32p.so (packed f32x2)
 Up-to-date outputs (newer than every source they depend on) are skipped.  Processes not listed here are generated and
 compiled by heget_process_create at first use (needs nvcc at run time).
 (`ptxas -O1` halves the compile time of the big processes but costs 10-35 % of their speed -- measured, not used.)
@@ -38,6 +38,11 @@ PROCESSES = [
     "u u > u u g",
     "u u~ > g g g g",
 ]
+
+
+# The packed-FP32 path (HEGET_FP32X2) is an experiment that did not pay: pre-built only for the two
+# processes its tests use; any other process is compiled on demand by heget_process_create.
+PACKED_PROCESSES = ["u u~ > g g", "g g > g g g"]
 
 
 def tag_of(process):
@@ -111,7 +116,8 @@ def build_kernels(processes=None, force=False, jobs=None, verbose=True):
         cu = os.path.join(KDIR, "gen_%s.cu" % tag)
         if force or not _newer(cu, [exe]):
             _run([exe, tag, proc, cu])
-        for prec, suf in ((0, "f64"), (1, "f32")):
+        precs = [(0, "f64"), (1, "f32")] + ([(2, "f32p")] if proc in PACKED_PROCESSES else [])
+        for prec, suf in precs:
             so = os.path.join(KDIR, "heget_%s_%s.so" % (tag, suf))
             if force or not _newer(so, [cu] + dev_sources()):
                 todo.append((cu, so, prec, n_legs(proc)))

@@ -78,7 +78,7 @@ heget_status_t open_plugin(const std::string& so, const std::string& key, const 
 // $HEGET_CACHE_DIR (default: the same kernels/ directory).
 heget_status_t load_plugin(const std::string& name, const std::string& tag, int n_legs, int prec, const hg::ProcDesc** out) {
     std::lock_guard<std::mutex> lock(g_mutex);
-    const std::string key = tag + (prec == 0 ? "_f64" : "_f32");
+    const std::string key = tag + (prec == 0 ? "_f64" : prec == 1 ? "_f32" : "_f32p");
     std::map<std::string, const hg::ProcDesc*>::iterator it = g_plugins.find(key);
     if (it != g_plugins.end()) { *out = it->second; return HEGET_OK; }
     const std::string dir = lib_dir() + "/kernels";
@@ -96,7 +96,7 @@ heget_status_t load_plugin(const std::string& name, const std::string& tag, int 
     if (rc != 0) return fail(HEGET_ECOMPILE, "generator failed for '%s': %s", name.c_str(), msg);
     const char* nvcc = getenv("HEGET_NVCC");
     const std::string cmd = std::string(nvcc ? nvcc : "nvcc") + " -std=c++17 -O3 -gencode arch=compute_100a,code=sm_100a -lineinfo -shared -Xcompiler -fPIC" +
-                            " -DHG_ONLY_PREC=" + (prec == 0 ? "0" : "1") + (n_legs >= 6 ? " -DHG_NO_LANES1" : "") + " -I'" + lib_dir() + "/csrc/device' -o '" + tmp +
+                            " -DHG_ONLY_PREC=" + (prec == 0 ? "0" : prec == 1 ? "1" : "2") + (n_legs >= 6 ? " -DHG_NO_LANES1" : "") + " -I'" + lib_dir() + "/csrc/device' -o '" + tmp +
                             "' '" + cu + "' > '" + log + "' 2>&1";
     if (system(cmd.c_str()) != 0) return fail(HEGET_ECOMPILE, "nvcc failed for '%s' (see %s)", name.c_str(), log.c_str());
     if (rename(tmp.c_str(), dst.c_str()) != 0) return fail(HEGET_ECOMPILE, "cannot install %s", dst.c_str());
@@ -165,9 +165,11 @@ heget_status_t heget_process_create(const char* process, double sqrt_s_hat, doub
     if (!process || !out) return fail(HEGET_EINVAL, "heget_process_create: NULL argument");
     if (!(sqrt_s_hat > 0.0) || !(alpha_s > 0.0) || !std::isfinite(sqrt_s_hat) || !std::isfinite(alpha_s))
         return fail(HEGET_EINVAL, "heget_process_create: sqrt_s_hat and alpha_s must be positive and finite");
-    if (prec != HEGET_FP64 && prec != HEGET_FP32) return fail(HEGET_EINVAL, "heget_process_create: unknown precision %d", (int)prec);
+    if (prec != HEGET_FP64 && prec != HEGET_FP32 && prec != HEGET_FP32X2) return fail(HEGET_EINVAL, "heget_process_create: unknown precision %d", (int)prec);
     std::string name, tag; int n_legs = 0;
     if (!canonical(process, name, tag, n_legs)) return fail(HEGET_EINVAL, "heget_process_create: cannot parse process '%s'", process);
+    if (prec == HEGET_FP32X2 && (" " + name + " ").find(" g ") == std::string::npos)
+        return fail(HEGET_EUNSUPPORTED, "process '%s' has no gluon whose two helicities could share a packed thread", name.c_str());
     const hg::ProcDesc* d = 0;
     heget_status_t st = load_plugin(name, tag, n_legs, (int)prec, &d);
     if (st != HEGET_OK) return st;
@@ -208,7 +210,7 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
     o->n_color = d->n_color; o->n_color_eval = d->n_color_eval; o->n_color_reduced = d->n_color_reduced;
     o->avg_spin = d->avg_spin; o->avg_color = d->avg_color; o->sym_factor = d->sym_factor;
     o->flops_per_event = d->flops_per_event; o->flops_per_helicity = d->flops_per_hel;
-    o->threads_per_block = d->block[p->prec]; o->lanes_wide = d->lanes_wide; o->lanes = effective_lanes(p);
+    o->threads_per_block = d->block[p->prec == HEGET_FP32 ? 1 : 0]; o->lanes_wide = d->lanes_wide; o->lanes = effective_lanes(p);
     o->regs_per_thread = -1; o->local_bytes_per_thread = -1;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {

@@ -24,6 +24,7 @@
 //    chirality sign chi (+1: left-handed line, -1: right-handed line) instead of cmplx[6] with two zero entries.
 // Metric (+,-,-,-); 4-vectors are (E, x, y, z) with UPPER indices; all momenta flow INTO the diagram.
 #pragma once
+#include <cstring>
 
 #if defined(__CUDACC__)
 #define HG_HD __host__ __device__ __forceinline__
@@ -46,6 +47,57 @@
 #endif
 
 namespace hg {
+
+// ------------------------------------------------------------------------------------------------------------------
+// f2: two FP32 values processed by one instruction (Blackwell FFMA2/FMUL2/FADD2 on a 64-bit register pair).  The packed
+// FP32 path instantiates the whole library with T = f2, the two halves being two helicity configurations of the same
+// event that differ in one gluon's helicity: every arithmetic instruction then does the work of two, which halves the
+// instruction count of the long straight-line bodies (they are instruction-fetch bound).
+// The operators are `mul/add/sub.f32x2` without a rounding modifier, so ptxas contracts a product and a sum into one
+// FFMA2 exactly as it does for scalar float (checked in the SASS).  Comparisons look at the first half: they are only
+// applied to values that are the same in both halves (chirality signs).
+// ------------------------------------------------------------------------------------------------------------------
+struct __align__(8) f2 {
+    unsigned long long v;             // both halves in one 64-bit register: low word = first configuration, high = second
+    f2() = default;
+    HG_HD static unsigned int bits(float a) {
+#if defined(__CUDA_ARCH__)
+        return __float_as_uint(a);
+#else
+        unsigned int u; memcpy(&u, &a, 4); return u;
+#endif
+    }
+    HG_HD static float val(unsigned int u) {
+#if defined(__CUDA_ARCH__)
+        return __uint_as_float(u);
+#else
+        float a; memcpy(&a, &u, 4); return a;
+#endif
+    }
+    HG_HD f2(float a, float b) : v(((unsigned long long)bits(b) << 32) | bits(a)) {}
+    HG_HD f2(float a) : f2(a, a) {}
+    HG_HD f2(double a) : f2((float)a, (float)a) {}
+    HG_HD f2(int a) : f2((float)a, (float)a) {}
+    HG_HD float lo() const { return val((unsigned int)v); }
+    HG_HD float hi() const { return val((unsigned int)(v >> 32)); }
+};
+#if defined(__CUDA_ARCH__)
+#define HG_F2_BODY(ptx, cexpr) { f2 r; asm(ptx " %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+#else
+#define HG_F2_BODY(ptx, cexpr) { return cexpr; }
+#endif
+HG_HD f2 operator+(f2 a, f2 b) HG_F2_BODY("add.f32x2", f2(a.lo() + b.lo(), a.hi() + b.hi()))
+HG_HD f2 operator-(f2 a, f2 b) HG_F2_BODY("sub.f32x2", f2(a.lo() - b.lo(), a.hi() - b.hi()))
+HG_HD f2 operator*(f2 a, f2 b) HG_F2_BODY("mul.f32x2", f2(a.lo() * b.lo(), a.hi() * b.hi()))
+#undef HG_F2_BODY
+HG_HD f2 operator-(f2 a) { f2 r; r.v = a.v ^ 0x8000000080000000ull; return r; }
+HG_HD f2& operator+=(f2& a, f2 b) { a = a + b; return a; }
+HG_HD f2& operator-=(f2& a, f2 b) { a = a - b; return a; }
+HG_HD f2& operator*=(f2& a, f2 b) { a = a * b; return a; }
+HG_HD bool operator>(f2 a, f2 b) { return a.lo() > b.lo(); }
+HG_HD bool operator<(f2 a, f2 b) { return a.lo() < b.lo(); }
+HG_HD bool operator>=(f2 a, f2 b) { return a.lo() >= b.lo(); }
+HG_HD bool operator==(f2 a, f2 b) { return a.lo() == b.lo(); }
 
 template <typename T> struct cx { T re, im; };
 template <typename T> struct vec4 { cx<T> v[4]; };     // gluon wavefunction / off-shell gluon current

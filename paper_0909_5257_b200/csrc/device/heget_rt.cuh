@@ -89,6 +89,33 @@ template <typename T> __device__ __forceinline__ void fence() {
 #endif
 #endif
 }
+template <> __device__ __forceinline__ f2 ldc<f2>(const f2* p) {          // same policy as an 8-byte scalar: never hoisted
+#if defined(HG_CACHE_HOISTABLE64)
+    return *p;
+#else
+    f2 r; r.v = *reinterpret_cast<const volatile unsigned long long*>(p); return r;
+#endif
+}
+// ---- packing of helicity configurations (1 per thread for float/double, 2 for f2) -----------------------------------
+// Packed threads hold the configurations t with gluon bit `pb` cleared (first half) and set (second half).
+template <typename T> struct hpack {
+    static constexpr int value = 1;
+    typedef T out_t;
+    __device__ static __forceinline__ int expand(int t, int) { return t; }
+    __device__ static __forceinline__ int index(int h, int) { return h; }
+    __device__ static __forceinline__ T select(int, int) { return T(1); }
+    __device__ static __forceinline__ T lam(int hidx, int j, int) { return ((hidx >> j) & 1) ? T(1) : T(-1); }
+    __device__ static __forceinline__ T hsum(T v) { return v; }
+};
+template <> struct hpack<f2> {
+    static constexpr int value = 2;
+    typedef float out_t;
+    __device__ static __forceinline__ int expand(int t, int pb) { return ((t >> pb) << (pb + 1)) | (t & ((1 << pb) - 1)); }
+    __device__ static __forceinline__ int index(int h, int pb) { return ((h >> (pb + 1)) << pb) | (h & ((1 << pb) - 1)); }
+    __device__ static __forceinline__ f2 select(int h, int pb) { return ((h >> pb) & 1) ? f2(0.f, 1.f) : f2(1.f, 0.f); }
+    __device__ static __forceinline__ f2 lam(int hidx, int j, int pb) { return j == pb ? f2(-1.f, 1.f) : (((hidx >> j) & 1) ? f2(1.f) : f2(-1.f)); }
+    __device__ static __forceinline__ float hsum(f2 v) { return v.lo() + v.hi(); }
+};
 template <typename T> __host__ __device__ constexpr bool leaf_reload() {
 #if defined(HG_LEAF_RELOAD32)
     return true;

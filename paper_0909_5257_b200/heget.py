@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libheget.so")
 
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM, ECOMPILE = range(6)
-FP64, FP32 = 0, 1
+FP64, FP32, FP32X2 = 0, 1, 2
 HEL_SUM, HEL_SAMPLE, HEL_FIXED = 0, 1, 2
 
 EXPORTS = ["heget_process_create", "heget_process_info", "heget_color_matrix", "heget_sample_momenta", "heget_eval_me2",
@@ -97,11 +97,11 @@ def _hptr(t, dtype, numel, name):
 
 
 class Process:
-    """heget_process_create / heget_destroy.  `precision` is "fp64" or "fp32"."""
+    """heget_process_create / heget_destroy.  `precision` is "fp64", "fp32" or "fp32x2" (FP32 on packed f32x2 instructions)."""
 
     def __init__(self, process, sqrt_s_hat, alpha_s=0.118, cuts=(20.0, 2.5, 0.4), precision="fp64"):
         self._h = None
-        self.precision = {"fp64": FP64, "fp32": FP32}[precision]
+        self.precision = {"fp64": FP64, "fp32": FP32, "fp32x2": FP32X2}[precision]
         self.dtype = torch.float64 if self.precision == FP64 else torch.float32
         c = Cuts(*cuts) if cuts is not None else None
         h = C.c_void_p()

@@ -129,6 +129,41 @@ def test_me2_fp32_matches_oracle(events, oracle_process, name, sqrt_s, seed, n):
     assert err.max() <= TOL32_MAX, "max rel err %.3e at event %d" % (err.max(), int(err.argmax()))
 
 
+@pytest.mark.parametrize("name,sqrt_s,seed,n", [c for c in CASES if c[0] in ("u u~ > g g", "g g > g g g")])
+def test_me2_fp32x2_matches_oracle(events, oracle_process, name, sqrt_s, seed, n):
+    """The packed path (two helicity configurations per thread on f32x2 instructions) is FP32 arithmetic: same tolerances; and
+    it must agree with the scalar FP32 path to FP32 rounding, event by event."""
+    mom, mom_h = events(name, sqrt_s, seed, n)
+    P = hg.Process(name, sqrt_s, precision="fp32x2")
+    ref = oracle_process(name).me2(mom_h)
+    for lanes in sorted({1, P.info.lanes_wide}):
+        try:
+            P.set_lanes(lanes)
+        except hg.HegetError as e:
+            assert e.status == hg.EINVAL and lanes == 1 and P.n_ext >= 6
+            continue
+        out = P.eval_me2(mom)
+        assert out.dtype == torch.float32
+        err = rel_err(out.cpu().numpy().astype(np.float64), ref)
+        assert np.all(np.isfinite(err))
+        assert np.median(err) <= TOL32_MEDIAN, "lanes %d: median rel err %.3e" % (lanes, np.median(err))
+        assert err.max() <= TOL32_MAX, "lanes %d: max rel err %.3e at event %d" % (lanes, err.max(), int(err.argmax()))
+    # single-configuration modes pick the right half of a packed pair
+    sub = mom[:, :, :64].contiguous()
+    total = torch.zeros(64, dtype=torch.float64, device="cuda")
+    for bits in range(1 << P.n_ext):
+        hel = [1 if (bits >> i) & 1 else -1 for i in range(P.n_ext)]
+        total += P.eval_me2(sub, mode=hg.HEL_FIXED, hel=hel).double()
+    full = P.eval_me2(sub).double()
+    assert ((total - full).abs() / full).max().item() < 1e-4
+
+
+def test_packed_needs_a_gluon():
+    with pytest.raises(hg.HegetError) as ei:
+        hg.Process("u u > u u", 500.0, precision="fp32x2")
+    assert ei.value.status == hg.EUNSUPPORTED
+
+
 def test_c1_closed_form(events):
     """C1 against the textbook result (BASELINE.json configs[0]): me2/S = g^4 [32/27 (t^2+u^2)/(tu) - 8/3 (t^2+u^2)/s^2]."""
     mom, m = events("u u~ > g g", 500.0, 0, 16384)
