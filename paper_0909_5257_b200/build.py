@@ -37,6 +37,7 @@ PROCESSES = [
     "u u~ > g g g",
     "u u > u u g",
     "u u~ > g g g g",
+    "u g > u g g",          # a crossing of u u~ > g g g
 ]
 
 

@@ -25,6 +25,7 @@ CASES = [
     ("u u > u u", 500.0, 6, 5003),
     ("u u~ > g g g", 1000.0, 7, 3001),
     ("u u > u u g", 1000.0, 8, 3001),
+    ("u g > u g g", 1000.0, 10, 3001),
     ("g g > g g g", 1000.0, 1, 8195),
     ("u u > u u g g", 1000.0, 2, 4099),
     ("u u~ > g g g g", 1500.0, 9, 1027),
@@ -162,6 +163,23 @@ def test_packed_needs_a_gluon():
     with pytest.raises(hg.HegetError) as ei:
         hg.Process("u u > u u", 500.0, precision="fp32x2")
     assert ei.value.status == hg.EUNSUPPORTED
+
+
+def test_runtime_generated_process(oracle_process, tmp_path, monkeypatch):
+    """A process that is not pre-built: heget_process_create runs the generator in-process, compiles its output with nvcc for
+    sm_100a, caches the plug-in (step a0 at run time) -- and the result matches the oracle like any other."""
+    import shutil
+    if shutil.which("nvcc") is None:
+        pytest.skip("no nvcc on this box: run-time generation returns HEGET_ECOMPILE")
+    monkeypatch.setenv("HEGET_CACHE_DIR", str(tmp_path))
+    name = "u d > u d g"
+    P = hg.Process(name, 1000.0)
+    assert (tmp_path / "heget_ud_udg_f64.so").exists()
+    assert (P.info.n_diagrams, P.info.n_color) == (5, 4)
+    mom = P.sample_momenta(12, 2003)
+    out = P.eval_me2(mom).cpu().numpy()
+    ref = oracle_process(name).me2(mom.cpu().numpy())
+    assert rel_err(out, ref).max() <= TOL64
 
 
 def test_c1_closed_form(events):
