@@ -28,10 +28,51 @@ struct EmitOptions {
 // flops of the device-library calls as written in heget_dev.cuh (FMA = 2, complex multiply = 6, complex add = 2)
 struct FlopTable {
     static int of_current(int kind) {
-        switch (kind) { case CK_GGG: return 157; case CK_GGGG: return 65; case CK_FUSE: return 42; case CK_FG: case CK_BG: return 74; default: return 0; }
+        switch (kind) { case CK_GGG: return 157; case CK_GGGG: return 65; case CK_FUSE: return 42; case CK_FG: case CK_BG: return 74; case CK_OPEN3: return 157; case CK_OPEN4: return 65; default: return 0; }
     }
-    static int of_closing(int kind) { switch (kind) { case AK_VVV: return 168; case AK_GGGG: return 70; default: return 58; } }
+    static int of_closing(int kind) { switch (kind) { case AK_VVV: return 168; case AK_GGGG: return 70; case AK_DOT: return 30; default: return 58; } }
 };
+
+// Closings that differ in ONE of their currents share the rest of the vertex: V3(a,b,c) = open3(a,b) . c (cyclic in a,b,c) and
+// W_piece(a,b,c,d) = open4(a,b,c;piece) . d, where open* is the off-shell current of that vertex without its propagator
+// (checked numerically against vvvxxx / ggggxxp).  A 3-leg sub-tree comes in several colour pieces, all closing on the same
+// partner currents: the open vertex is built once (150 flops) and every piece costs a 4-vector product (30 flops) instead of a
+// full vvvxxx (168).  The open vertices are ordinary nodes of the current graph, so the scheduler places them like any current.
+static inline void share_closings(Graph& G) {
+    typedef std::vector<int> Key;
+    std::map<Key, int> count;
+    for (size_t l = 0; l < G.closings.size(); ++l) {
+        const Closing& cl = G.closings[l];
+        if (cl.kind == AK_VVV) for (int r = 0; r < 3; ++r) { Key k; k.push_back(0); k.push_back(cl.c[r]); k.push_back(cl.c[(r + 1) % 3]); count[k]++; }
+        else if (cl.kind == AK_GGGG) { Key k; k.push_back(1); k.push_back(cl.c[0]); k.push_back(cl.c[1]); k.push_back(cl.c[2]); k.push_back(cl.piece); count[k]++; }
+    }
+    std::map<Key, int> made;
+    for (size_t l = 0; l < G.closings.size(); ++l) {
+        Closing& cl = G.closings[l];
+        Key best; int bestn = 1, rest = -1;
+        if (cl.kind == AK_VVV) {
+            for (int r = 0; r < 3; ++r) { Key k; k.push_back(0); k.push_back(cl.c[r]); k.push_back(cl.c[(r + 1) % 3]); if (count[k] > bestn) { bestn = count[k]; best = k; rest = cl.c[(r + 2) % 3]; } }
+        } else if (cl.kind == AK_GGGG) {
+            Key k; k.push_back(1); k.push_back(cl.c[0]); k.push_back(cl.c[1]); k.push_back(cl.c[2]); k.push_back(cl.piece);
+            if (count[k] > bestn) { bestn = count[k]; best = k; rest = cl.c[3]; }
+        }
+        if (rest < 0) continue;
+        if (!made.count(best)) {
+            Cur W; W.id = (int)G.cur.size(); W.ptype = PT_G; W.end_leg = -1; W.leg = -1; W.piece = best[0] ? best[4] : 0;
+            W.kind = best[0] ? CK_OPEN4 : CK_OPEN3;
+            W.ch[0] = best[1]; W.ch[1] = best[2]; W.ch[2] = best[0] ? best[3] : -1;
+            W.mask = 0; W.varmask = 0; W.size = 0;
+            for (int j = 0; j < 3; ++j) if (W.ch[j] >= 0) {
+                const Cur& c = G.cur[W.ch[j]];
+                W.mask |= c.mask; W.varmask |= c.varmask; W.size += c.size;
+                for (size_t q = 0; q < c.pairs.size(); ++q) W.pairs.push_back(c.pairs[q]);
+            }
+            std::sort(W.pairs.begin(), W.pairs.end());
+            made[best] = W.id; G.cur.push_back(W);
+        }
+        cl.kind = AK_DOT; cl.c[0] = made[best]; cl.c[1] = rest; cl.c[2] = cl.c[3] = -1;
+    }
+}
 
 struct Emitter {
     const Graph& G;
@@ -171,7 +212,7 @@ struct Emitter {
                 for (size_t m = 0; m < miss.size(); ++m) for (int j = 0; j < 3; ++j) { const int ch = G.cur[miss[m]].ch[j]; if (ch >= 0) { if (!tmp[ch]) touched.push_back(ch); tmp[ch]++; } }
                 for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) { const int ch = cl.c[j]; if (!tmp[ch]) touched.push_back(ch); tmp[ch]++; }
                 int born = 0, dying = 0, closest = 255;
-                for (size_t m = 0; m < miss.size(); ++m) if (uses[miss[m]] - tmp[miss[m]] > 0) ++born;          // new and still needed afterwards
+                for (size_t m = 0; m < miss.size(); ++m) if (uses[miss[m]] - tmp[miss[m]] > 0 && G.cur[miss[m]].kind != CK_OPEN3 && G.cur[miss[m]].kind != CK_OPEN4) ++born;   // new and still needed afterwards (open vertices are short-lived helpers of the currents already alive: not charged)
                 for (size_t q = 0; q < touched.size(); ++q) {
                     const int ch = touched[q];
                     if (G.cur[ch].kind == CK_LEAF || !done[ch]) continue;

@@ -61,7 +61,7 @@ static inline Process parse_process(const std::string& text) {
 }
 
 enum PType { PT_G = 0, PT_F = 1, PT_B = 2 };                      // gluon, psi (holds an in-end), psibar (holds an out-end)
-enum CKind { CK_LEAF = 0, CK_GGG, CK_GGGG, CK_FUSE, CK_FG, CK_BG }; // jvvxx0, jgggx0, jioxx0, fvixx0, fvoxx0
+enum CKind { CK_LEAF = 0, CK_GGG, CK_GGGG, CK_FUSE, CK_FG, CK_BG, CK_OPEN3, CK_OPEN4 };   // OPEN*: vertex with one leg left open, no propagator // jvvxx0, jgggx0, jioxx0, fvixx0, fvoxx0
 
 struct Cur {
     int id; unsigned mask; int size;
@@ -72,7 +72,7 @@ struct Cur {
     CExpr colour;
 };
 
-enum AKind { AK_VVV = 0, AK_GGGG, AK_IOV };
+enum AKind { AK_VVV = 0, AK_GGGG, AK_IOV, AK_DOT };   // DOT: (open vertex, wavefunction) Minkowski product
 struct Closing {
     int kind, piece;
     int c[4];                         // current ids; AK_IOV: (psibar, psi, gluon)

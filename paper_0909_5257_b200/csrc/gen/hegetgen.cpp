@@ -1,5 +1,5 @@
 // hegetgen: the host-side process generator of heget-b200.
-//   hegetgen <tag> "<process>" <out.cu> [--block64 N] [--block32 N] [--jreg64 N] [--jreg32 N]
+//   hegetgen <tag> "<process>" <out.cu> [--block64 N] [--block32 N] [--jreg64 N] [--jreg32 N] [--share-closings 0|1]
 // writes one specialised CUDA source for the process and prints a one-line summary (counts of Table 1).
 //   hegetgen --summary "<process>"      prints the counts and the distinct colour-matrix values (Table 4)
 #include <cstdio>
@@ -25,18 +25,20 @@ int main(int argc, char** argv) {
             return 0;
         }
         if (argc < 4) { fprintf(stderr, "usage: hegetgen <tag> \"<process>\" <out.cu> [options]\n"); return 2; }
-        EmitOptions opt;
+        EmitOptions opt; bool share = false;
         for (int i = 4; i + 1 < argc; i += 2) {
             if (!strcmp(argv[i], "--block64")) opt.block64 = atoi(argv[i + 1]);
             else if (!strcmp(argv[i], "--block32")) opt.block32 = atoi(argv[i + 1]);
             else if (!strcmp(argv[i], "--jreg64")) opt.jreg_max64 = atoi(argv[i + 1]);
             else if (!strcmp(argv[i], "--jreg32")) opt.jreg_max32 = atoi(argv[i + 1]);
+            else if (!strcmp(argv[i], "--share-closings")) share = atoi(argv[i + 1]) != 0;
             else { fprintf(stderr, "unknown option %s\n", argv[i]); return 2; }
         }
         Process P = parse_process(argv[2]);
         // the kernel sums diagrams on the minimal (Fierzed) basis; for two quark lines the paper's over-complete
         // basis (reading A12) is built as well, for n_color and the colour matrix of Table 4
         Graph G; G.build(P, false);
+        if (share) share_closings(G);      // experiment, off by default: fewer flops but 2x the live currents
         Graph GP; const Graph* paper = 0;
         if (two_lines(P)) { GP.build(P, true); paper = &GP; }
         Emitter E(G, argv[1], opt);
