@@ -46,6 +46,13 @@ typedef enum {
  * Needs at least one external gluon (the two configurations differ in its helicity), else HEGET_EUNSUPPORTED. */
 typedef enum { HEGET_FP64 = 0, HEGET_FP32 = 1, HEGET_FP32X2 = 2 } heget_precision_t;
 
+/* Kernel back end of steps a3-a8.  STRAIGHT: one specialised kernel per process whose helicity body is
+ * straight-line code written by the generator and compiled by nvcc (pre-built for the configured processes, else compiled
+ * at heget_process_create).  TABLE: generic kernels that interpret the process's table program -- merged sub-currents,
+ * closings at the centroid vertex, every sub-current computed once per helicity assignment of its own legs and reused by
+ * all configurations (no compiler needed).  AUTO: TABLE for processes with >= 6 external legs, STRAIGHT below. */
+typedef enum { HEGET_KERNEL_AUTO = 0, HEGET_KERNEL_STRAIGHT = 1, HEGET_KERNEL_TABLE = 2 } heget_kernel_t;
+
 /* helicity treatment of eq. 12.  SUM: all 2^n_ext configurations (the graded mode, reading A8).
  * SAMPLE: one configuration per event drawn from Philox(seed, global event index), weighted by 2^n_ext -- what the paper
  * itself ran.  FIXED: the single configuration given in `hel` (no weight). */
@@ -64,6 +71,8 @@ typedef struct {
     int n_color;               /* colour-basis size in the paper's convention (Table 1)                           */
     int n_color_eval;          /* size of the basis the kernel accumulates J on                                   */
     int n_color_reduced;       /* after merging elements whose J are proportional for every phase-space point     */
+    int n_color_accum;         /* dimension J is accumulated on: the span of the diagrams' colour vectors (TABLE), else = n_color_reduced */
+    int color_rank;            /* rank of the n_color x n_color colour matrix of eq. 9 (A13: 12 of 40 for u u -> u u g g); -1 if not computed */
     double avg_spin;           /* 1/4                       (eq. 12)                                              */
     double avg_color;          /* 1/(n_a n_b)               (eq. 9)                                               */
     double sym_factor;         /* 1/prod k!                                         */
@@ -74,6 +83,9 @@ typedef struct {
     int threads_per_block;
     int lanes_wide;            /* helicity lanes per event of the wide kernel variant (see heget_set_lanes)        */
     int lanes;                 /* lanes per event of the variant currently selected                               */
+    int kernel;                /* back end the next heget_eval_me2 takes: HEGET_KERNEL_STRAIGHT or HEGET_KERNEL_TABLE */
+    int events_per_block;
+    double flops_per_event_tensor; /* flops of the colour stage executed on the tensor pipe (0: vector pipes)        */
 } heget_info_t;
 
 /* Build (or look up) the specialised kernels of one process.
@@ -91,7 +103,8 @@ heget_status_t heget_process_create(const char* process, double sqrt_s_hat, doub
 heget_status_t heget_process_info(const heget_process_t* proc, heget_info_t* out);
 
 /* Colour matrix C of eq. 9 WITHOUT the 1/(n_a n_b) average, row-major.
- *   which = 0: n_color x n_color in the paper's basis (Tables 1 and 4);  which = 1: the reduced matrix the kernel contracts.
+ *   which = 0: n_color x n_color in the paper's basis (Tables 1 and 4);  which = 1: the reduced (merged-basis) matrix;
+ *   which = 2: the n_color_accum x n_color_accum congruence B^T C B the TABLE kernels contract (STRAIGHT: same as 1).
  * h_out may be NULL to query the dimension only; *n receives the dimension. */
 heget_status_t heget_color_matrix(const heget_process_t* proc, int which, double* h_out, int* n);
 
@@ -116,7 +129,8 @@ heget_status_t heget_eval_me2(heget_process_t* proc, const double* d_mom, uint64
                               const int8_t* hel, uint64_t seed, uint64_t first_event, void* d_me2, void* cuda_stream);
 
 /* The same two steps with HOST buffers: the library stages through a device scratch it owns (grown on demand, freed by
- * heget_destroy), copies on `cuda_stream` and synchronises it before returning.  h_me2 is double[] or float[] per the
+ * heget_destroy), copies on `cuda_stream` and synchronises it before returning; calls on ONE handle from several host
+ * threads are serialised by the library (the scratch belongs to the handle).  h_me2 is double[] or float[] per the
  * handle's precision.  Either of h_mom_in / h_mom_out may be NULL:
  *   heget_run_host(.., h_mom_in = NULL, ..)  samples (seed, first_event) on the device, evaluates, returns me2 (and the
  *                                            momenta / weights if h_mom_out / h_weight are non-NULL);
@@ -125,7 +139,11 @@ heget_status_t heget_run_host(heget_process_t* proc, uint64_t seed, uint64_t fir
                               const double* h_mom_in, double* h_mom_out, double* h_weight, heget_hel_mode_t mode,
                               const int8_t* hel, void* h_me2, void* cuda_stream);
 
-/* Choose the kernel variant: `lanes` threads share one event and split its helicity configurations among them.
+/* Choose the kernel back end (see heget_kernel_t).  Builds or loads what the choice needs (HEGET_ECOMPILE /
+ * HEGET_EUNSUPPORTED as for heget_process_create; the previous choice stays on failure).  HEGET_FP32X2 handles are STRAIGHT only. */
+heget_status_t heget_set_kernel(heget_process_t* proc, heget_kernel_t kernel);
+
+/* STRAIGHT back end only (TABLE accepts 0 and nothing else).  Choose the kernel variant: `lanes` threads share one event and split its helicity configurations among them.
  * 0 = automatic (FP64: the wide variant, FP32: one event per thread where built, else wide; wide = info.lanes_wide = the largest power of two <= 32 dividing n_hel_eval, so a warp works
  * on 32/lanes events, event-cache reads are broadcasts and the per-event prologue is spread over the lanes);
  * 1 = one event per thread (not built for processes with >= 6 legs); lanes_wide = the wide variant. Else HEGET_EINVAL. */

@@ -25,13 +25,12 @@ LIB = os.path.join(HERE, "libheget.so")
 NVCC = os.environ.get("HEGET_NVCC", "nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo"]
 
-# BASELINE.json configs C1..C5 first, then the small processes the parity tests use
+# BASELINE.json configs C1..C4 first (C5: SLOW_PROCESSES), then the small processes the parity tests use
 PROCESSES = [
     "u u~ > g g",
     "g g > g g g",
     "u u > u u g g",
     "g g > g g g g",
-    "u u~ > g g g g g",
     "g g > g g",
     "u u > u u",
     "u u~ > g g g",
@@ -40,6 +39,10 @@ PROCESSES = [
     "u g > u g g",          # a crossing of u u~ > g g g
 ]
 
+
+# The straight-line kernels of the 7-leg config take ~10 minutes of ptxas per precision; the table back end (no compilation)
+# is what serves processes with >= 6 legs, so they are only built on request: `python -m paper_0909_5257_b200.build --slow`.
+SLOW_PROCESSES = ["u u~ > g g g g g"]
 
 # The packed-FP32 path (HEGET_FP32X2) is an experiment that did not pay: pre-built only for the two
 # processes its tests use; any other process is compiled on demand by heget_process_create.
@@ -144,6 +147,7 @@ if __name__ == "__main__":
     ap = argparse.ArgumentParser()
     ap.add_argument("--only", nargs="*", help="process strings to build (default: the configured list)")
     ap.add_argument("--force", action="store_true")
+    ap.add_argument("--slow", action="store_true", help="also build the straight-line kernels of SLOW_PROCESSES")
     ap.add_argument("--jobs", type=int, default=None)
     a = ap.parse_args()
-    print(build_all(a.only or None, a.force, a.jobs))
+    print(build_all(a.only or (PROCESSES + SLOW_PROCESSES if a.slow else None), a.force, a.jobs))

@@ -15,8 +15,11 @@
 #include <unistd.h>
 #include "../../include/heget.h"
 #include "rambo.cuh"
+#include "device/heget_tab.cuh"
+#include "gen/tabprog.hpp"
 
 extern "C" int heget_generate_source(const char* tag, const char* process, const char* out_path, char* msg, int msglen);
+heget::TabProgram* heget_build_table(const char* tag, const char* process, int* rc, char* msg, int msglen);
 
 namespace {
 
@@ -63,15 +66,22 @@ bool canonical(const char* process, std::string& name, std::string& tag, int& n_
     return !toks.empty();
 }
 
-heget_status_t open_plugin(const std::string& so, const std::string& key, const hg::ProcDesc** out) {
+heget_status_t open_plugin(const std::string& so, const std::string& key, const std::string& name, const hg::ProcDesc** out) {
     void* h = dlopen(so.c_str(), RTLD_NOW | RTLD_LOCAL);
     if (!h) return fail(HEGET_ECOMPILE, "dlopen %s: %s", so.c_str(), dlerror());
     typedef const hg::ProcDesc* (*fn_t)();
     fn_t fn = (fn_t)dlsym(h, "heget_plugin_desc");
-    if (!fn) return fail(HEGET_ECOMPILE, "%s exports no heget_plugin_desc", so.c_str());
-    *out = g_plugins[key] = fn();
+    if (!fn) { dlclose(h); return fail(HEGET_ECOMPILE, "%s exports no heget_plugin_desc", so.c_str()); }
+    const hg::ProcDesc* d = fn();
+    // a plug-in built against other headers, or one whose tag aliases another process, is refused, not misread
+    if (!d || d->abi_version != HG_ABI_VERSION) { dlclose(h); return fail(HEGET_ECOMPILE, "%s was built for another version of the library: rebuild it (python -m paper_0909_5257_b200.build)", so.c_str()); }
+    if (name != d->name) { dlclose(h); return fail(HEGET_EINVAL, "process '%s' is not the canonical spelling of '%s'", name.c_str(), d->name); }
+    *out = g_plugins[key] = d;
     return HEGET_OK;
 }
+
+// single-quote a string for /bin/sh
+std::string shq(const std::string& v) { std::string o = "'"; for (size_t i = 0; i < v.size(); ++i) { if (v[i] == '\'') o += "'\\''"; else o += v[i]; } return o + "'"; }
 
 // One plug-in per (process, precision): kernels/heget_<tag>_f64.so / _f32.so beside this library, built ahead of time by
 // paper_0909_5257_b200/build.py for the configured processes, else generated and compiled here (step a0) and cached in
@@ -84,30 +94,35 @@ heget_status_t load_plugin(const std::string& name, const std::string& tag, int 
     const std::string dir = lib_dir() + "/kernels";
     const char* cache = getenv("HEGET_CACHE_DIR");
     const std::string wdir = cache ? std::string(cache) : dir;
-    if (exists(dir + "/heget_" + key + ".so")) return open_plugin(dir + "/heget_" + key + ".so", key, out);
+    if (exists(dir + "/heget_" + key + ".so")) return open_plugin(dir + "/heget_" + key + ".so", key, name, out);
     const std::string dst = wdir + "/heget_" + key + ".so";
-    if (exists(dst)) return open_plugin(dst, key, out);
+    if (exists(dst)) return open_plugin(dst, key, name, out);
     mkdir(wdir.c_str(), 0755);
-    const std::string cu = wdir + "/gen_" + tag + ".cu", log = wdir + "/gen_" + key + ".log", tmp = dst + ".tmp";
+    // intermediate files carry the pid: ranks that build the same process at the same time do not share them, and the
+    // finished plug-in is moved into place atomically
+    const std::string uniq = key + "." + std::to_string((long)getpid());
+    const std::string cu = wdir + "/gen_" + uniq + ".cu", log = wdir + "/gen_" + uniq + ".log", tmp = dst + "." + std::to_string((long)getpid()) + ".tmp";
     char msg[512] = "";
     const int rc = heget_generate_source(tag.c_str(), name.c_str(), cu.c_str(), msg, sizeof msg);
     if (rc == 1) return fail(HEGET_EINVAL, "process '%s': %s", name.c_str(), msg);
     if (rc == 2) return fail(HEGET_EUNSUPPORTED, "process '%s': %s", name.c_str(), msg);
     if (rc != 0) return fail(HEGET_ECOMPILE, "generator failed for '%s': %s", name.c_str(), msg);
     const char* nvcc = getenv("HEGET_NVCC");
-    const std::string cmd = std::string(nvcc ? nvcc : "nvcc") + " -std=c++17 -O3 -gencode arch=compute_100a,code=sm_100a -lineinfo -shared -Xcompiler -fPIC" +
-                            " -DHG_ONLY_PREC=" + (prec == 0 ? "0" : prec == 1 ? "1" : "2") + (n_legs >= 6 ? " -DHG_NO_LANES1" : "") + " -I'" + lib_dir() + "/csrc/device' -o '" + tmp +
-                            "' '" + cu + "' > '" + log + "' 2>&1";
+    const std::string cmd = shq(nvcc ? nvcc : "nvcc") + " -std=c++17 -O3 -gencode arch=compute_100a,code=sm_100a -lineinfo -shared -Xcompiler -fPIC" +
+                            " -DHG_ONLY_PREC=" + (prec == 0 ? "0" : prec == 1 ? "1" : "2") + (n_legs >= 6 ? " -DHG_NO_LANES1" : "") + " -I" + shq(lib_dir() + "/csrc/device") + " -o " + shq(tmp) +
+                            " " + shq(cu) + " > " + shq(log) + " 2>&1";
     if (system(cmd.c_str()) != 0) return fail(HEGET_ECOMPILE, "nvcc failed for '%s' (see %s)", name.c_str(), log.c_str());
     if (rename(tmp.c_str(), dst.c_str()) != 0) return fail(HEGET_ECOMPILE, "cannot install %s", dst.c_str());
-    return open_plugin(dst, key, out);
+    unlink(cu.c_str());
+    return open_plugin(dst, key, name, out);
 }
 
-double rambo_flat_weight(int n, double sqrt_s) {      // reading A7: (pi/2)^(n-1) s^(n-2) / ((n-1)!(n-2)!) (2 pi)^(4-3n)
-    const double PI = 3.14159265358979323846;
-    double w = pow(PI / 2.0, n - 1) * pow(sqrt_s * sqrt_s, n - 2) * pow(2.0 * PI, 4 - 3 * n);
-    for (int k = 2; k <= n - 1; ++k) w /= (double)k;
-    for (int k = 2; k <= n - 2; ++k) w /= (double)k;
+// flat n-body massless phase-space volume (reading A7): V_n = (pi/2)^(n-1) s^(n-2) / ((n-1)! (n-2)!), times (2 pi)^(4-3n).
+// Accumulated body by body: V_2 (2 pi)^-2 = 1/(8 pi), and every further particle multiplies by (pi/2) s / ((k-1)(k-2)) / (2 pi)^3.
+double flat_phase_space_weight(int n, double sqrt_s) {
+    const double pi = acos(-1.0), s = sqrt_s * sqrt_s;
+    double w = 1.0 / (8.0 * pi);
+    for (int k = 3; k <= n; ++k) w *= (pi / 2.0) * s / ((double)(k - 1) * (double)(k - 2)) / (8.0 * pi * pi * pi);
     return w;
 }
 
@@ -127,14 +142,28 @@ __global__ void __launch_bounds__(256) k_fma_probe(T* out, unsigned long long it
 struct heget_process;
 static int effective_lanes(const heget_process* p);
 
+// One handle = one process at one precision.  Two kernel back ends can serve it (heget_set_kernel):
+//   d   : the straight-line plug-in (one specialised kernel per process, generated source compiled by nvcc), loaded on demand
+//   tab : the table program interpreted by the generic kernels of device/heget_tab.cuh (built in-process, no compiler)
 struct heget_process {
     const hg::ProcDesc* d;
+    heget::TabProgram* tab;
+    hg::TabDev tdev; bool tab_on_device; std::vector<void*> tab_allocs; int tab_epc;
+    std::string name, tag;
+    int n_legs, kernel_req;        // requested back end: HEGET_KERNEL_AUTO / STRAIGHT / TABLE
     int prec, lanes;
     double sqrt_s, alpha_s, out_scale;
     heget_cuts_t cuts;
-    // scratch of the host-buffer entry point
-    double* s_mom; double* s_w; void* s_me2; size_t s_cap;
+    // scratch of the host-buffer entry point; s_mutex serialises heget_run_host calls on one handle
+    double* s_mom; double* s_w; void* s_me2; size_t s_cap; std::mutex s_mutex;
 };
+
+// which back end a call takes: the table program for processes with >= 6 legs (their straight-line kernels are 1-3 MB of
+// code and instruction-fetch bound), the specialised straight-line kernel below that
+static int effective_kernel(const heget_process* p) {
+    if (p->kernel_req != HEGET_KERNEL_AUTO) return p->kernel_req;
+    return p->n_legs >= 6 ? HEGET_KERNEL_TABLE : HEGET_KERNEL_STRAIGHT;
+}
 
 // lanes = 0 (automatic): FP64 takes the wide variant (event-cache reads become warp broadcasts; measured 26 vs 23 TFLOP/s on
 // C2), FP32 the one-event-per-thread variant where it is built (the compiler keeps the event cache in registers across the
@@ -142,6 +171,90 @@ struct heget_process {
 static int effective_lanes(const heget_process* p) {
     if (p->lanes) return p->lanes;
     return (p->prec == HEGET_FP32 && (p->d->lanes_avail & 1)) ? 1 : p->d->lanes_wide;
+}
+
+// ---- the two back ends, loaded on demand -----------------------------------------------------------------------------------
+static heget_status_t need_plugin(heget_process* p) {
+    if (p->d) return HEGET_OK;
+    return load_plugin(p->name, p->tag, p->n_legs, p->prec, &p->d);
+}
+static heget_status_t need_table(heget_process* p) {
+    if (p->tab) return HEGET_OK;
+    if (p->prec == HEGET_FP32X2) return fail(HEGET_EUNSUPPORTED, "the packed-FP32 precision exists for the straight-line kernels only");
+    char msg[512] = ""; int rc = 3;
+    p->tab = heget_build_table(p->tag.c_str(), p->name.c_str(), &rc, msg, sizeof msg);
+    if (rc == 1) return fail(HEGET_EINVAL, "process '%s': %s", p->name.c_str(), msg);
+    if (rc == 2) return fail(HEGET_EUNSUPPORTED, "process '%s': %s", p->name.c_str(), msg);
+    if (rc != 0 || !p->tab) return fail(HEGET_ECOMPILE, "generator failed for '%s': %s", p->name.c_str(), msg);
+    return HEGET_OK;
+}
+static heget_status_t need_backend(heget_process* p) { return effective_kernel(p) == HEGET_KERNEL_TABLE ? need_table(p) : need_plugin(p); }
+
+template <typename V> static heget_status_t upload(heget_process* p, const std::vector<V>& v, const V** out) {
+    void* dptr = 0;
+    const size_t bytes = (v.size() ? v.size() : 1) * sizeof(V);
+    if (cudaMalloc(&dptr, bytes) != cudaSuccess) { cudaGetLastError(); return fail(HEGET_ENOMEM, "cannot allocate %zu bytes of device memory for the process tables", bytes); }
+    p->tab_allocs.push_back(dptr);
+    if (v.size()) CU(cudaMemcpy(dptr, v.data(), v.size() * sizeof(V), cudaMemcpyHostToDevice));
+    *out = (const V*)dptr;
+    return HEGET_OK;
+}
+
+// events per CTA of the table kernels: the choice with the most resident warps per SM (shared memory and 2048 threads bound it)
+template <typename T> static int tab_pick_epc(const hg::TabDev& d, size_t* smem_out) {
+    int best = 1; long best_warps = -1;
+    for (int epc = 1; epc <= 8; ++epc) {
+        const int threads = epc * d.nchunks * 32;
+        if (threads > 256) break;
+        const size_t smem = hg::tab_smem_bytes<T>(d, epc) + 32;
+        if (smem > 227 * 1024) break;
+        long ctas = std::min<long>(std::min<long>((long)((228 * 1024) / (smem + 1024)), 32), 2048 / threads);
+        const long warps = ctas * epc * d.nchunks;
+        if (warps > best_warps) { best_warps = warps; best = epc; }
+    }
+    if (smem_out) *smem_out = hg::tab_smem_bytes<T>(d, best) + 32;
+    return best_warps < 0 ? 0 : best;
+}
+
+static heget_status_t table_to_device(heget_process* p) {
+    if (p->tab_on_device) return HEGET_OK;
+    const heget::TabProgram& t = *p->tab;
+    hg::TabDev& d = p->tdev;
+    memset(&d, 0, sizeof d);
+    d.n_ext = t.n_ext; d.NH = t.NH; d.nchunks = t.nchunks; d.cpc = t.cpc; d.R = t.R; d.Rpad = t.Rpad; d.nK = t.nK; d.store32 = t.store32;
+    d.n_levels = t.n_levels; d.n_closings = t.n_closings;
+    heget_status_t st;
+    if ((st = upload(p, t.kmask, &d.kmask)) != HEGET_OK) return st;
+    if ((st = upload(p, t.leginfo, &d.leginfo)) != HEGET_OK) return st;
+    if ((st = upload(p, t.a_hdr, &d.a_hdr)) != HEGET_OK) return st;
+    if ((st = upload(p, t.a_out, &d.a_out)) != HEGET_OK) return st;
+    if ((st = upload(p, t.a_term, &d.a_term)) != HEGET_OK) return st;
+    if ((st = upload(p, t.a_level, &d.a_level)) != HEGET_OK) return st;
+    if ((st = upload(p, t.b_entry, &d.b_entry)) != HEGET_OK) return st;
+    if ((st = upload(p, t.b_vtab, &d.b_vtab)) != HEGET_OK) return st;
+    if ((st = upload(p, t.jl_index, &d.jl_index)) != HEGET_OK) return st;
+    if ((st = upload(p, t.jl_coef, &d.jl_coef)) != HEGET_OK) return st;
+    if ((st = upload(p, t.evalidx, &d.evalidx)) != HEGET_OK) return st;
+    if (p->prec == HEGET_FP64) {
+        const double* c = 0; if ((st = upload(p, t.cmat, &c)) != HEGET_OK) return st; d.cmat = c;
+        if ((st = upload(p, t.coef, &c)) != HEGET_OK) return st; d.coef = c;
+    } else {
+        std::vector<float> cm(t.cmat.begin(), t.cmat.end()), cf(t.coef.begin(), t.coef.end()); const float* c = 0;
+        if ((st = upload(p, cm, &c)) != HEGET_OK) return st; d.cmat = c;
+        if ((st = upload(p, cf, &c)) != HEGET_OK) return st; d.coef = c;
+    }
+    size_t smem = 0;
+    p->tab_epc = p->prec == HEGET_FP64 ? tab_pick_epc<double>(d, &smem) : tab_pick_epc<float>(d, &smem);
+    if (p->tab_epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
+    if (p->prec == HEGET_FP64) CU(cudaFuncSetAttribute(hg::k_tab<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else CU(cudaFuncSetAttribute(hg::k_tab<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    p->tab_on_device = true;
+    return HEGET_OK;
+}
+
+static void table_free_device(heget_process* p) {
+    for (size_t i = 0; i < p->tab_allocs.size(); ++i) cudaFree(p->tab_allocs[i]);
+    p->tab_allocs.clear(); p->tab_on_device = false;
 }
 
 extern "C" {
@@ -170,17 +283,19 @@ heget_status_t heget_process_create(const char* process, double sqrt_s_hat, doub
     if (!canonical(process, name, tag, n_legs)) return fail(HEGET_EINVAL, "heget_process_create: cannot parse process '%s'", process);
     if (prec == HEGET_FP32X2 && (" " + name + " ").find(" g ") == std::string::npos)
         return fail(HEGET_EUNSUPPORTED, "process '%s' has no gluon whose two helicities could share a packed thread", name.c_str());
-    const hg::ProcDesc* d = 0;
-    heget_status_t st = load_plugin(name, tag, n_legs, (int)prec, &d);
-    if (st != HEGET_OK) return st;
     heget_process* p = new (std::nothrow) heget_process();
     if (!p) return fail(HEGET_ENOMEM, "out of host memory");
-    p->d = d; p->prec = (int)prec; p->lanes = 0; p->sqrt_s = sqrt_s_hat; p->alpha_s = alpha_s;
+    p->d = 0; p->tab = 0; p->tab_on_device = false; p->tab_epc = 0; p->name = name; p->tag = tag; p->n_legs = n_legs;
+    p->kernel_req = prec == HEGET_FP32X2 ? HEGET_KERNEL_STRAIGHT : HEGET_KERNEL_AUTO;
+    p->prec = (int)prec; p->lanes = 0; p->sqrt_s = sqrt_s_hat; p->alpha_s = alpha_s;
     p->cuts.pt_min = cuts ? cuts->pt_min : 0.0; p->cuts.eta_max = cuts ? cuts->eta_max : 0.0; p->cuts.dr_min = cuts ? cuts->dr_min : 0.0;
+    p->s_mom = 0; p->s_w = 0; p->s_me2 = 0; p->s_cap = 0;
+    const heget_status_t st = need_backend(p);
+    if (st != HEGET_OK) { delete p; return st; }
     // S * 1/4 * 1/(n_a n_b) * g_s^(2(n-2)) * s_hat^-(n-4): the kernels work in units of sqrt(s_hat) (reading A21)
     const double gs2 = 4.0 * 3.14159265358979323846 * alpha_s;
-    p->out_scale = d->sym_factor * d->avg_spin * d->avg_color * pow(gs2, d->n_ext - 2) * pow(sqrt_s_hat, -2.0 * (d->n_ext - 4));
-    p->s_mom = 0; p->s_w = 0; p->s_me2 = 0; p->s_cap = 0;
+    const double sym = p->tab ? p->tab->sym_factor : p->d->sym_factor, avs = p->tab ? p->tab->avg_spin : p->d->avg_spin, avc = p->tab ? p->tab->avg_color : p->d->avg_color;
+    p->out_scale = sym * avs * avc * pow(gs2, n_legs - 2) * pow(sqrt_s_hat, -2.0 * (n_legs - 4));
     *out = p;
     return HEGET_OK;
 }
@@ -190,11 +305,28 @@ void heget_destroy(heget_process_t* p) {
     if (p->s_mom) cudaFree(p->s_mom);
     if (p->s_w) cudaFree(p->s_w);
     if (p->s_me2) cudaFree(p->s_me2);
+    table_free_device(p);
+    delete p->tab;
     delete p;
+}
+
+heget_status_t heget_set_kernel(heget_process_t* p, heget_kernel_t kernel) {
+    if (!p) return fail(HEGET_EINVAL, "heget_set_kernel: NULL handle");
+    if (kernel != HEGET_KERNEL_AUTO && kernel != HEGET_KERNEL_STRAIGHT && kernel != HEGET_KERNEL_TABLE) return fail(HEGET_EINVAL, "heget_set_kernel: unknown back end %d", (int)kernel);
+    if (p->prec == HEGET_FP32X2 && kernel == HEGET_KERNEL_TABLE) return fail(HEGET_EUNSUPPORTED, "the packed-FP32 precision exists for the straight-line kernels only");
+    const int old = p->kernel_req;
+    p->kernel_req = p->prec == HEGET_FP32X2 ? HEGET_KERNEL_STRAIGHT : (int)kernel;
+    const heget_status_t st = need_backend(p);
+    if (st != HEGET_OK) p->kernel_req = old;
+    return st;
 }
 
 heget_status_t heget_set_lanes(heget_process_t* p, int lanes) {
     if (!p) return fail(HEGET_EINVAL, "heget_set_lanes: NULL handle");
+    if (effective_kernel(p) == HEGET_KERNEL_TABLE) {
+        if (lanes != 0 && lanes != 32) return fail(HEGET_EINVAL, "heget_set_lanes: the table kernels have one layout (a warp per 32 helicity configurations); lanes must be 0 or 32");
+        p->lanes = 0; return HEGET_OK;
+    }
     const hg::ProcDesc* d = p->d;
     const bool ok = lanes == 0 || (lanes == 1 && (d->lanes_avail & 1)) || (lanes == d->lanes_wide && (d->lanes_avail & 2));
     if (!ok) return fail(HEGET_EINVAL, "heget_set_lanes: lanes = %d is not built for '%s' (0 = automatic%s, wide = %d)", lanes, d->name,
@@ -204,26 +336,57 @@ heget_status_t heget_set_lanes(heget_process_t* p, int lanes) {
 
 heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
     if (!p || !o) return fail(HEGET_EINVAL, "heget_process_info: NULL argument");
-    const hg::ProcDesc* d = p->d;
     memset(o, 0, sizeof *o);
+    o->regs_per_thread = -1; o->local_bytes_per_thread = -1; o->color_rank = -1;
+    int ndev = 0;
+    const bool have_dev = cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0;
+    if (!have_dev) cudaGetLastError();
+    if (effective_kernel(p) == HEGET_KERNEL_TABLE) {
+        const heget::TabProgram& t = *p->tab;
+        o->kernel = HEGET_KERNEL_TABLE;
+        o->n_ext = t.n_ext; o->n_hel = t.n_hel; o->n_hel_eval = t.NH; o->n_diagrams = t.n_diagrams; o->n_topologies = t.n_topologies;
+        o->n_color = t.n_color; o->n_color_eval = t.n_color_eval; o->n_color_reduced = t.NJ; o->n_color_accum = t.R; o->color_rank = t.color_rank;
+        o->avg_spin = t.avg_spin; o->avg_color = t.avg_color; o->sym_factor = t.sym_factor;
+        o->flops_per_event = t.flops_per_event; o->flops_per_helicity = t.flops_per_hel;
+        o->lanes_wide = 32; o->lanes = 32;
+        hg::TabDev d; memset(&d, 0, sizeof d); d.n_ext = t.n_ext; d.nchunks = t.nchunks; d.R = t.R; d.nK = t.nK; d.store32 = t.store32;
+        const int epc = p->prec == HEGET_FP64 ? tab_pick_epc<double>(d, 0) : tab_pick_epc<float>(d, 0);
+        o->events_per_block = epc; o->threads_per_block = epc * t.nchunks * 32;
+        if (have_dev) {
+            cudaFuncAttributes fa;
+            const cudaError_t e = p->prec == HEGET_FP64 ? cudaFuncGetAttributes(&fa, hg::k_tab<double>) : cudaFuncGetAttributes(&fa, hg::k_tab<float>);
+            if (e == cudaSuccess) { o->regs_per_thread = fa.numRegs; o->local_bytes_per_thread = (int)fa.localSizeBytes; } else cudaGetLastError();
+        }
+        return HEGET_OK;
+    }
+    const hg::ProcDesc* d = p->d;
+    o->kernel = HEGET_KERNEL_STRAIGHT;
     o->n_ext = d->n_ext; o->n_hel = d->n_hel; o->n_hel_eval = d->n_hel_eval; o->n_diagrams = d->n_diagrams; o->n_topologies = d->n_topologies;
-    o->n_color = d->n_color; o->n_color_eval = d->n_color_eval; o->n_color_reduced = d->n_color_reduced;
+    o->n_color = d->n_color; o->n_color_eval = d->n_color_eval; o->n_color_reduced = d->n_color_reduced; o->n_color_accum = d->n_color_reduced;
+    if (p->tab) o->color_rank = p->tab->color_rank;
     o->avg_spin = d->avg_spin; o->avg_color = d->avg_color; o->sym_factor = d->sym_factor;
     o->flops_per_event = d->flops_per_event; o->flops_per_helicity = d->flops_per_hel;
-    o->threads_per_block = d->block[p->prec == HEGET_FP32 ? 1 : 0]; o->lanes_wide = d->lanes_wide; o->lanes = effective_lanes(p);
-    o->regs_per_thread = -1; o->local_bytes_per_thread = -1;
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0) {
+    o->threads_per_block = d->block[p->prec == HEGET_FP64 ? 0 : 1]; o->lanes_wide = d->lanes_wide; o->lanes = effective_lanes(p);
+    o->events_per_block = o->threads_per_block / o->lanes;
+    if (have_dev) {
         hg::KernelInfo ki;
-        if (d->kernel_info(p->prec, effective_lanes(p), &ki) == 0) { o->regs_per_thread = ki.regs; o->local_bytes_per_thread = ki.local_bytes; o->threads_per_block = ki.block; }
+        if (d->kernel_info(p->prec, effective_lanes(p), &ki) == 0) { o->regs_per_thread = ki.regs; o->local_bytes_per_thread = ki.local_bytes; o->threads_per_block = ki.block; o->events_per_block = ki.block / o->lanes; }
         else cudaGetLastError();
-    } else cudaGetLastError();
+    }
     return HEGET_OK;
 }
 
 heget_status_t heget_color_matrix(const heget_process_t* p, int which, double* h_out, int* n) {
     if (!p || !n) return fail(HEGET_EINVAL, "heget_color_matrix: NULL argument");
-    if (which != 0 && which != 1) return fail(HEGET_EINVAL, "heget_color_matrix: which must be 0 or 1");
+    if (which < 0 || which > 2) return fail(HEGET_EINVAL, "heget_color_matrix: which must be 0, 1 or 2");
+    if (effective_kernel(p) == HEGET_KERNEL_TABLE) {
+        const heget::TabProgram& t = *p->tab;
+        const std::vector<double>& c = which == 0 ? t.colour_paper : which == 1 ? t.colour_red : t.colour_acc;
+        const int m = which == 0 ? t.n_color : which == 1 ? t.NJ : t.R;
+        *n = m;
+        if (h_out) memcpy(h_out, c.data(), sizeof(double) * (size_t)m * m);
+        return HEGET_OK;
+    }
     const int m = which == 0 ? p->d->n_color : p->d->n_color_reduced;
     *n = m;
     if (h_out) memcpy(h_out, which == 0 ? p->d->colour_matrix : p->d->colour_matrix_eval, sizeof(double) * (size_t)m * m);
@@ -236,10 +399,10 @@ heget_status_t heget_sample_momenta(heget_process_t* p, uint64_t seed, uint64_t 
     if (n_events == 0) return HEGET_OK;
     if (!d_mom) return fail(HEGET_EINVAL, "heget_sample_momenta: d_mom is NULL");
     if (n_events > (1ull << 31) * 128ull) return fail(HEGET_EINVAL, "heget_sample_momenta: n_events too large");
-    const int nf = p->d->n_ext - 2;
+    const int nf = p->n_legs - 2;
     hg::RamboArgs a;
     a.sqrt_s = p->sqrt_s; a.pt_min = p->cuts.pt_min; a.eta_max = p->cuts.eta_max; a.dr_min = p->cuts.dr_min;
-    a.w0 = rambo_flat_weight(nf, p->sqrt_s);
+    a.w0 = flat_phase_space_weight(nf, p->sqrt_s);
     a.seed = seed; a.first_event = first_event; a.n_events = n_events; a.mom = d_mom; a.weight = d_weight; a.tries = d_tries;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const unsigned int blocks = (unsigned int)((n_events + 127) / 128);
@@ -263,22 +426,46 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
     if (mode == HEGET_HEL_FIXED && !hel) return fail(HEGET_EINVAL, "heget_eval_me2: HEL_FIXED needs hel");
     if (n_events == 0) return HEGET_OK;
     if (!d_mom || !d_me2) return fail(HEGET_EINVAL, "heget_eval_me2: NULL device pointer");
+    const bool table = effective_kernel(p) == HEGET_KERNEL_TABLE;
+    const int n_ext = p->n_legs;
+    const int n_eval = table ? p->tab->NH : p->d->n_hel_eval;
+    const signed char* htab = table ? (const signed char*)p->tab->hel_table.data() : p->d->hel_table;
+    int hel_fixed = -1;
+    if (mode == HEGET_HEL_FIXED) {
+        for (int i = 0; i < n_ext; ++i) if (hel[i] != 1 && hel[i] != -1) return fail(HEGET_EINVAL, "heget_eval_me2: hel[%d] = %d is not +-1", i, (int)hel[i]);
+        for (int h = 0; h < n_eval && hel_fixed < 0; ++h) {
+            bool same = true;
+            for (int i = 0; i < n_ext; ++i) if (htab[h * n_ext + i] != hel[i]) { same = false; break; }
+            if (same) hel_fixed = h;
+        }
+    }
+    if (table) {
+        const heget_status_t st = table_to_device(p);
+        if (st != HEGET_OK) return st;
+        const int epc = p->tab_epc;
+        const unsigned long long blocks = (n_events + epc - 1) / epc;
+        if (blocks > 0x7fffffffull) return fail(HEGET_EINVAL, "heget_eval_me2: n_events too large for one launch");
+        const int threads = epc * p->tdev.nchunks * 32;
+        cudaStream_t s = (cudaStream_t)cuda_stream;
+        if (p->prec == HEGET_FP64) {
+            const size_t smem = hg::tab_smem_bytes<double>(p->tdev, epc) + 32;
+            hg::k_tab<double><<<(unsigned int)blocks, threads, smem, s>>>(p->tdev, epc, d_mom, n_events, 1.0 / p->sqrt_s, p->out_scale, (double*)d_me2, (int)mode, hel_fixed, seed, first_event);
+        } else {
+            const size_t smem = hg::tab_smem_bytes<float>(p->tdev, epc) + 32;
+            hg::k_tab<float><<<(unsigned int)blocks, threads, smem, s>>>(p->tdev, epc, d_mom, n_events, 1.0 / p->sqrt_s, p->out_scale, (float*)d_me2, (int)mode, hel_fixed, seed, first_event);
+        }
+        CU(cudaGetLastError());
+        g_launches++;
+        return HEGET_OK;
+    }
     const hg::ProcDesc* d = p->d;
     hg::LaunchArgs a;
     a.d_mom = d_mom; a.n_events = n_events; a.inv_sqrt_s = 1.0 / p->sqrt_s; a.out_scale = p->out_scale; a.d_me2 = d_me2;
-    a.hel_mode = (int)mode; a.hel_fixed = -1; a.seed = seed; a.first_event = first_event; a.d_jbuf = 0; a.lanes = effective_lanes(p);
+    a.hel_mode = (int)mode; a.hel_fixed = hel_fixed; a.seed = seed; a.first_event = first_event; a.lanes = effective_lanes(p);
     // one configuration per event: in the wide variant all lanes of an event would evaluate the same configuration, so take
     // the one-event-per-thread variant where it is built (the big processes only have the wide one: L-fold redundant there)
     if (mode != HEGET_HEL_SUM && p->lanes == 0 && (d->lanes_avail & 1)) a.lanes = 1;
     a.stream = (cudaStream_t)cuda_stream;
-    if (mode == HEGET_HEL_FIXED) {
-        for (int i = 0; i < d->n_ext; ++i) if (hel[i] != 1 && hel[i] != -1) return fail(HEGET_EINVAL, "heget_eval_me2: hel[%d] = %d is not +-1", i, (int)hel[i]);
-        for (int h = 0; h < d->n_hel_eval && a.hel_fixed < 0; ++h) {
-            bool same = true;
-            for (int i = 0; i < d->n_ext; ++i) if (d->hel_table[h * d->n_ext + i] != hel[i]) { same = false; break; }
-            if (same) a.hel_fixed = h;
-        }
-    }
     const int rc = d->launch(p->prec, a);
     if (rc != 0) return fail(HEGET_ECUDA, "launch of '%s' failed: %s", d->name, cudaGetErrorString((cudaError_t)rc));
     g_launches++;
@@ -291,7 +478,8 @@ heget_status_t heget_run_host(heget_process_t* p, uint64_t seed, uint64_t first_
     if (!p) return fail(HEGET_EINVAL, "heget_run_host: NULL handle");
     if (n_events == 0) return HEGET_OK;
     if (!h_me2) return fail(HEGET_EINVAL, "heget_run_host: h_me2 is NULL");
-    const size_t nm = (size_t)p->d->n_ext * 4 * n_events, esz = p->prec == HEGET_FP64 ? 8 : 4;
+    std::lock_guard<std::mutex> lock(p->s_mutex);      // the device scratch belongs to the handle: one host call at a time
+    const size_t nm = (size_t)p->n_legs * 4 * n_events, esz = p->prec == HEGET_FP64 ? 8 : 4;
     if (p->s_cap < n_events) {
         if (p->s_mom) cudaFree(p->s_mom); if (p->s_w) cudaFree(p->s_w); if (p->s_me2) cudaFree(p->s_me2);
         p->s_mom = 0; p->s_w = 0; p->s_me2 = 0; p->s_cap = 0;

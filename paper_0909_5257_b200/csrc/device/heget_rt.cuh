@@ -20,7 +20,6 @@ struct LaunchArgs {
     int hel_fixed;            // mode 2: index of the configuration in the kernel's own enumeration, or -1 (vanishing)
     uint64_t seed;            // mode 1
     uint64_t first_event;     // mode 1: global index of event 0 (Philox counter)
-    void* d_jbuf;             // colour-GEMM variant: J chunk [2*NJ][columns], else NULL
     int lanes;                // helicity lanes per event (power of two <= 32), 0 = choose
     cudaStream_t stream;
 };
@@ -52,7 +51,9 @@ struct ProcDesc {
     int lanes_wide;             // helicity lanes per event of the wide variant (power of two <= 32 dividing n_hel_eval)
     int lanes_avail;            // bit 0: the one-event-per-thread variant is compiled in, bit 1: the wide variant is
     ProcDesc* next;
+    int abi_version;            // HG_ABI_VERSION of the headers the plug-in was compiled against (checked at load)
 };
+#define HG_ABI_VERSION 2
 
 // every plug-in (one shared object per process) exports   extern "C" const hg::ProcDesc* heget_plugin_desc();
 

@@ -61,7 +61,10 @@ static inline Process parse_process(const std::string& text) {
 }
 
 enum PType { PT_G = 0, PT_F = 1, PT_B = 2 };                      // gluon, psi (holds an in-end), psibar (holds an out-end)
-enum CKind { CK_LEAF = 0, CK_GGG, CK_GGGG, CK_FUSE, CK_FG, CK_BG, CK_OPEN3, CK_OPEN4 };   // OPEN*: vertex with one leg left open, no propagator // jvvxx0, jgggx0, jioxx0, fvixx0, fvoxx0
+enum CKind { CK_LEAF = 0, CK_GGG, CK_GGGG, CK_FUSE, CK_FG, CK_BG, CK_OPEN3, CK_OPEN4, CK_SUM };   // OPEN*: vertex with one leg left open, no propagator // jvvxx0, jgggx0, jioxx0, fvixx0, fvoxx0
+
+// one vertex evaluation inside a merged current (CK_SUM): coef * vertex_kind(ch...) ; the propagator is applied to the sum
+struct Term { int kind, ch[3], piece; Frac coef; };
 
 struct Cur {
     int id; unsigned mask; int size;
@@ -70,6 +73,8 @@ struct Cur {
     std::vector<std::pair<int, int> > pairs;   // completed quark lines (in-end, out-end) inside
     unsigned varmask;                 // legs whose helicity/chirality bit selects the variant
     CExpr colour;
+    std::vector<Term> terms;          // CK_SUM only
+    double n_diag, n_topo;            // Feynman sub-diagrams summed in this current (Table 1 convention / plain topologies)
 };
 
 enum AKind { AK_VVV = 0, AK_GGGG, AK_IOV, AK_DOT };   // DOT: (open vertex, wavefunction) Minkowski product
@@ -86,6 +91,15 @@ struct Graph {
     Process P;
     int root;
     bool paper_basis;
+    // merge = true: currents over the same legs whose colour factors are proportional (a four-gluon piece and the pair of
+    // three-gluon vertices with the same f.f structure, eq. 36/40) are summed into ONE stored current
+    // (kind CK_SUM, one Term per vertex evaluation).  By linearity of every vertex in each of its legs the sum over diagrams
+    // (eq. 7) is unchanged; the parents and closings are then built from the merged currents only.
+    bool merge = false;
+    // centroid = true: diagrams are closed at their centroid vertex, so no current over more than n/2 legs is needed
+    // (default: at the vertex of the root leg, re-rooted when the other side of a cubic root vertex is a single leg: <= n-3 legs)
+    bool centroid = false;
+    double n_diagrams_paper = 0;
     ColourAlgebra ca;
     std::vector<Cur> cur;
     std::map<unsigned, std::vector<int> > by_mask;
@@ -171,9 +185,11 @@ struct Graph {
             if (L.type == LEG_G) { c.ptype = PT_G; c.end_leg = -1; c.colour = ca.leaf_gluon(leg); }
             else if (L.type == LEG_QIN) { c.ptype = PT_F; c.end_leg = leg; c.colour = ca.leaf_psi(leg); }
             else { c.ptype = PT_B; c.end_leg = leg; c.colour = ca.leaf_psibar(leg); }
+            c.n_diag = 1.0; c.n_topo = 1.0;
             add(c);
             return by_mask[S];
         }
+        std::vector<Cur> raws;
         for (int k = 2; k <= 3; ++k) {
             std::vector<std::vector<unsigned> > sp; splits(S, k, sp);
             for (size_t s = 0; s < sp.size(); ++s) {
@@ -186,15 +202,51 @@ struct Graph {
                     std::vector<int> ch(k); for (int j = 0; j < k; ++j) ch[j] = lists[j][idx[j]];
                     for (int piece = 0; piece < (k == 3 ? 3 : 1); ++piece) {
                         Cur c;
-                        if (combine(ch, c, piece)) { colour_of(c); add(c); }
+                        if (combine(ch, c, piece)) {
+                            colour_of(c);
+                            c.n_diag = 1.0; c.n_topo = (c.kind == CK_GGGG) ? 1.0 / 3.0 : 1.0;
+                            for (int q = 0; q < 3; ++q) if (c.ch[q] >= 0) { c.n_diag *= cur[c.ch[q]].n_diag; c.n_topo *= cur[c.ch[q]].n_topo; }
+                            if (merge) raws.push_back(c); else add(c);
+                        }
                     }
                     int j = k - 1; while (j >= 0 && ++idx[j] == lists[j].size()) { idx[j] = 0; --j; }
                     if (j < 0) break;
                 }
             }
         }
+        if (merge) merge_raws(raws);
         return by_mask[S];
     }
+
+    // group the raw currents over one leg set by (type, open end, completed quark lines, normalised colour) and store one
+    // CK_SUM current per group; raw currents whose colour vanishes identically are dropped
+    void merge_raws(std::vector<Cur>& raws) {
+        typedef std::pair<std::pair<std::pair<int, int>, std::vector<std::pair<int, int> > >, CExpr> Key;
+        std::map<Key, int> index;
+        std::vector<int> order;
+        for (size_t r = 0; r < raws.size(); ++r) {
+            Cur& c = raws[r];
+            if (c.colour.empty()) continue;
+            std::sort(c.pairs.begin(), c.pairs.end());
+            const Frac lead = c.colour.begin()->second, inv(lead.d, lead.n);
+            Key key; key.first.first = std::make_pair(c.ptype, c.end_leg); key.first.second = c.pairs; key.second = scaled(c.colour, inv);
+            Term t; t.kind = c.kind; t.piece = c.piece; for (int q = 0; q < 3; ++q) t.ch[q] = c.ch[q];
+            std::map<Key, int>::iterator it = index.find(key);
+            if (it == index.end()) {
+                Cur m = c; m.kind = CK_SUM; m.ch[0] = m.ch[1] = m.ch[2] = -1; m.piece = 0; m.terms.clear();
+                t.coef = Frac(1); m.terms.push_back(t);
+                const int id = add(m);
+                index[key] = id; order.push_back(id);
+                lead_of[id] = lead;
+            } else {
+                Cur& m = cur[it->second];
+                const Frac l0 = lead_of[it->second];
+                t.coef = lead * Frac(l0.d, l0.n);
+                m.terms.push_back(t); m.n_diag += c.n_diag; m.n_topo += c.n_topo;
+            }
+        }
+    }
+    std::map<int, Frac> lead_of;
 
     static int perm_sign(std::vector<std::pair<int, int> > pairs) {
         std::sort(pairs.begin(), pairs.end());
@@ -236,6 +288,7 @@ struct Graph {
     double topo_weight_of(int id) const {
         const Cur& c = cur[id];
         if (c.kind == CK_LEAF) return 1.0;
+        if (c.kind == CK_SUM) return c.n_topo;
         double w = (c.kind == CK_GGGG) ? 1.0 / 3.0 : 1.0;
         for (int j = 0; j < 3; ++j) if (c.ch[j] >= 0) w *= topo_weight_of(c.ch[j]);
         return w;
@@ -257,6 +310,20 @@ struct Graph {
         std::map<CTerm, int> basis_index;
         std::vector<CExpr> colours;
         const int max_part = std::max(1, n - 3);
+        if (centroid) {
+            // every tree has a vertex all of whose branches hold at most n/2 legs; when a branch holds exactly n/2 the vertex
+            // at its other end qualifies too, and the one on the root's side is taken: each diagram is closed exactly once
+            for (int k = 3; k <= 4; ++k) {
+                std::vector<std::vector<unsigned> > sp; splits(all, k, sp);
+                for (size_t s = 0; s < sp.size(); ++s) {
+                    bool ok = true;
+                    for (int j = 0; j < k; ++j) { const int sz = popcount(sp[s][j]); if (2 * sz > n || (2 * sz == n && (sp[s][j] & rbit))) ok = false; }
+                    if (!ok) continue;
+                    std::vector<unsigned> parts(sp[s].begin(), sp[s].end() - 1);
+                    close_parts(parts, sp[s].back(), basis_index, colours);
+                }
+            }
+        } else {
         // (i) the root alone + a 2- or 3-way split of the other legs, every part <= n-3 legs
         for (int k = 2; k <= 3; ++k) {
             std::vector<std::vector<unsigned> > sp; splits(rest, k, sp);
@@ -276,6 +343,7 @@ struct Graph {
                 for (size_t s = 0; s < sp.size(); ++s) close_parts(sp[s], pair, basis_index, colours);
             }
         }
+        }
         if (closings.empty()) throw std::invalid_argument("no tree-level QCD diagram for this process");
         // basis = every distinct colour structure that occurs (single traces / quark strings), in canonical order
         int m = 0;
@@ -285,8 +353,8 @@ struct Graph {
             Closing& cl = closings[l];
             for (CExpr::const_iterator it = colours[l].begin(); it != colours[l].end(); ++it)
                 cl.coef.push_back(std::make_pair(basis_index[it->first], it->second * Frac(cl.fermi_sign)));
-            double w = cl.topo_weight; for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) w *= topo_weight_of(cl.c[j]);
-            n_topologies += w;
+            double w = cl.topo_weight, nd = 1.0; for (int j = 0; j < 4; ++j) if (cl.c[j] >= 0) { w *= topo_weight_of(cl.c[j]); nd *= cur[cl.c[j]].n_diag; }
+            n_topologies += w; n_diagrams_paper += nd;
         }
         std::vector<int> gl; for (int i = 0; i < n; ++i) if (P.legs[i].type == LEG_G) gl.push_back(i);
         C.assign((size_t)m * m, Frac(0));

@@ -16,8 +16,10 @@ OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM, ECOMPILE = range(6)
 FP64, FP32, FP32X2 = 0, 1, 2
 HEL_SUM, HEL_SAMPLE, HEL_FIXED = 0, 1, 2
 
+KERNEL_AUTO, KERNEL_STRAIGHT, KERNEL_TABLE = 0, 1, 2
+
 EXPORTS = ["heget_process_create", "heget_process_info", "heget_color_matrix", "heget_sample_momenta", "heget_eval_me2",
-           "heget_run_host", "heget_set_lanes", "heget_fma_probe", "heget_destroy", "heget_last_error", "heget_launch_count"]
+           "heget_run_host", "heget_set_lanes", "heget_set_kernel", "heget_fma_probe", "heget_destroy", "heget_last_error", "heget_launch_count"]
 
 
 class HegetError(RuntimeError):
@@ -32,10 +34,11 @@ class Cuts(C.Structure):
 
 class Info(C.Structure):
     _fields_ = [("n_ext", C.c_int), ("n_hel", C.c_int), ("n_hel_eval", C.c_int), ("n_diagrams", C.c_int),
-                ("n_topologies", C.c_int), ("n_color", C.c_int), ("n_color_eval", C.c_int), ("n_color_reduced", C.c_int),
+                ("n_topologies", C.c_int), ("n_color", C.c_int), ("n_color_eval", C.c_int), ("n_color_reduced", C.c_int), ("n_color_accum", C.c_int), ("color_rank", C.c_int),
                 ("avg_spin", C.c_double), ("avg_color", C.c_double), ("sym_factor", C.c_double),
                 ("flops_per_event", C.c_double), ("flops_per_helicity", C.c_double),
-                ("regs_per_thread", C.c_int), ("local_bytes_per_thread", C.c_int), ("threads_per_block", C.c_int), ("lanes_wide", C.c_int), ("lanes", C.c_int)]
+                ("regs_per_thread", C.c_int), ("local_bytes_per_thread", C.c_int), ("threads_per_block", C.c_int), ("lanes_wide", C.c_int), ("lanes", C.c_int),
+                ("kernel", C.c_int), ("events_per_block", C.c_int), ("flops_per_event_tensor", C.c_double)]
 
 
 _lib = None
@@ -58,6 +61,7 @@ def lib():
         L.heget_eval_me2.argtypes = [vp, vp, u64, C.c_int, vp, u64, u64, vp, vp]
         L.heget_run_host.argtypes = [vp, u64, u64, u64, vp, vp, vp, C.c_int, vp, vp, vp]
         L.heget_set_lanes.argtypes = [vp, C.c_int]
+        L.heget_set_kernel.argtypes = [vp, C.c_int]
         L.heget_fma_probe.argtypes = [C.c_int, u64, vp, u64, C.POINTER(C.c_double), vp]
         L.heget_destroy.argtypes = [vp]
         L.heget_destroy.restype = None
@@ -99,7 +103,7 @@ def _hptr(t, dtype, numel, name):
 class Process:
     """heget_process_create / heget_destroy.  `precision` is "fp64", "fp32" or "fp32x2" (FP32 on packed f32x2 instructions)."""
 
-    def __init__(self, process, sqrt_s_hat, alpha_s=0.118, cuts=(20.0, 2.5, 0.4), precision="fp64"):
+    def __init__(self, process, sqrt_s_hat, alpha_s=0.118, cuts=(20.0, 2.5, 0.4), precision="fp64", kernel=None):
         self._h = None
         self.precision = {"fp64": FP64, "fp32": FP32, "fp32x2": FP32X2}[precision]
         self.dtype = torch.float64 if self.precision == FP64 else torch.float32
@@ -109,6 +113,8 @@ class Process:
                                           C.byref(c) if c is not None else None, self.precision, C.byref(h)))
         self._h = h
         self.process, self.sqrt_s_hat, self.alpha_s = process, float(sqrt_s_hat), float(alpha_s)
+        if kernel is not None:
+            _check(lib().heget_set_kernel(self._h, {"auto": KERNEL_AUTO, "straight": KERNEL_STRAIGHT, "table": KERNEL_TABLE}[kernel]))
         self.info = self.process_info()
         self.n_ext = self.info.n_ext
 
@@ -134,6 +140,11 @@ class Process:
         m = torch.zeros(n.value, n.value, dtype=torch.float64)
         _check(lib().heget_color_matrix(self._h, which, C.c_void_p(m.data_ptr()), C.byref(n)))
         return m
+
+    def set_kernel(self, kernel):
+        """heget_set_kernel: "auto", "straight" (specialised compiled kernel) or "table" (generic table-driven kernels)."""
+        _check(lib().heget_set_kernel(self._h, {"auto": KERNEL_AUTO, "straight": KERNEL_STRAIGHT, "table": KERNEL_TABLE}[kernel]))
+        self.info = self.process_info()
 
     def set_lanes(self, lanes):
         _check(lib().heget_set_lanes(self._h, int(lanes)))
