@@ -139,6 +139,7 @@ __global__ void __launch_bounds__(256) k_fma_probe(T* out, unsigned long long it
 
 }  // namespace
 
+struct TabShape { int epc, jm, tm_cols, tm_wcols; size_t smem; long warps; };
 struct heget_process;
 static int effective_lanes(const heget_process* p);
 
@@ -148,9 +149,10 @@ static int effective_lanes(const heget_process* p);
 struct heget_process {
     const hg::ProcDesc* d;
     heget::TabProgram* tab;
-    hg::TabDev tdev; bool tab_on_device; std::vector<void*> tab_allocs; int tab_epc;
+    hg::TabDev tdev; bool tab_on_device; std::vector<void*> tab_allocs; int tab_epc; TabShape tab_shape;
     std::string name, tag;
     int n_legs, kernel_req;        // requested back end: HEGET_KERNEL_AUTO / STRAIGHT / TABLE
+    bool auto_table;               // what AUTO means for this process
     int prec, lanes;
     double sqrt_s, alpha_s, out_scale;
     heget_cuts_t cuts;
@@ -158,11 +160,11 @@ struct heget_process {
     double* s_mom; double* s_w; void* s_me2; size_t s_cap; std::mutex s_mutex;
 };
 
-// which back end a call takes: the table program for processes with >= 6 legs (their straight-line kernels are 1-3 MB of
-// code and instruction-fetch bound), the specialised straight-line kernel below that
+// which back end a call takes.  AUTO: the table program for the big processes (>= 6 legs and >= 4 gluons: hundreds of
+// diagrams, whose straight-line kernels are 1-3 MB of code and instruction-fetch bound), the specialised kernel otherwise
 static int effective_kernel(const heget_process* p) {
     if (p->kernel_req != HEGET_KERNEL_AUTO) return p->kernel_req;
-    return p->n_legs >= 6 ? HEGET_KERNEL_TABLE : HEGET_KERNEL_STRAIGHT;
+    return p->auto_table ? HEGET_KERNEL_TABLE : HEGET_KERNEL_STRAIGHT;
 }
 
 // lanes = 0 (automatic): FP64 takes the wide variant (event-cache reads become warp broadcasts; measured 26 vs 23 TFLOP/s on
@@ -200,20 +202,49 @@ template <typename V> static heget_status_t upload(heget_process* p, const std::
     return HEGET_OK;
 }
 
-// events per CTA of the table kernels: the choice with the most resident warps per SM (shared memory and 2048 threads bound it)
-template <typename T> static int tab_pick_epc(const hg::TabDev& d, size_t* smem_out) {
-    int best = 1; long best_warps = -1;
-    for (int epc = 1; epc <= 8; ++epc) {
-        const int threads = epc * d.nchunks * 32;
-        if (threads > 256) break;
-        const size_t smem = hg::tab_smem_bytes<T>(d, epc) + 32;
-        if (smem > 227 * 1024) break;
-        long ctas = std::min<long>(std::min<long>((long)((228 * 1024) / (smem + 1024)), 32), 2048 / threads);
-        const long warps = ctas * epc * d.nchunks;
-        if (warps > best_warps) { best_warps = warps; best = epc; }
+// Launch shape of the table kernels: events per CTA and where J lives (shared memory, or tensor memory = TMEM), chosen for the
+// most resident warps per SM.  Bounds: shared memory, registers (regs per thread of the compiled kernel, 0 = unknown), 2048
+// threads, and for TMEM the 512 columns of an SM (a CTA allocates a power of two >= 32; the warps of a CTA that share a
+// 32-lane quadrant split the columns).  HEGET_TAB_J=smem|tmem forces the choice (experiments).
+template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, int regs_smem, int regs_tmem) {
+    TabShape best; best.epc = 0; best.jm = 0; best.tm_cols = 0; best.tm_wcols = 0; best.smem = 0; best.warps = -1;
+    const char* force = getenv("HEGET_TAB_J");
+    for (int jm = 0; jm < 2; ++jm) {
+        if (force && ((jm == 0) != (strcmp(force, "smem") == 0))) continue;
+        const int regs = jm ? regs_tmem : regs_smem;
+        const long reg_warps = regs > 0 ? 65536 / (((regs + 7) / 8 * 8) * 32) : 64;
+        for (int epc = 1; epc <= 8; ++epc) {
+            const int w = epc * d.nchunks, threads = w * 32;
+            if (threads > 256) break;
+            const size_t smem = hg::tab_smem_bytes<T>(d, epc, jm == 1) + 48;
+            if (smem > 227 * 1024) break;
+            long ctas = std::min<long>(std::min<long>((long)((228 * 1024) / (smem + 1024)), 32), 2048 / threads);
+            ctas = std::min<long>(ctas, reg_warps / w);
+            int cols = 0, wcols = 0;
+            if (jm) {
+                wcols = (int)(sizeof(T) / 4) * 2 * d.Rpad;
+                const int need = ((w + 3) / 4) * wcols;
+                cols = 32; while (cols < need) cols *= 2;
+                if (cols > 512) continue;
+                ctas = std::min<long>(ctas, 512 / cols);
+            }
+            const long warps = ctas * w;
+            if (warps > best.warps) { best.epc = epc; best.jm = jm; best.tm_cols = cols; best.tm_wcols = wcols; best.smem = smem; best.warps = warps; }
+        }
     }
-    if (smem_out) *smem_out = hg::tab_smem_bytes<T>(d, best) + 32;
-    return best_warps < 0 ? 0 : best;
+    return best;
+}
+
+template <typename T, int JM> static int tab_kernel_regs() {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return 0; }
+    cudaFuncAttributes fa;
+    if (cudaFuncGetAttributes(&fa, hg::k_tab<T, JM>) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return fa.numRegs;
+}
+static TabShape tab_shape_of(const hg::TabDev& d, int prec) {
+    return prec == HEGET_FP64 ? tab_pick_shape<double>(d, tab_kernel_regs<double, 0>(), tab_kernel_regs<double, 1>())
+                              : tab_pick_shape<float>(d, tab_kernel_regs<float, 0>(), tab_kernel_regs<float, 1>());
 }
 
 static heget_status_t table_to_device(heget_process* p) {
@@ -230,10 +261,42 @@ static heget_status_t table_to_device(heget_process* p) {
     if ((st = upload(p, t.a_out, &d.a_out)) != HEGET_OK) return st;
     if ((st = upload(p, t.a_term, &d.a_term)) != HEGET_OK) return st;
     if ((st = upload(p, t.a_level, &d.a_level)) != HEGET_OK) return st;
-    if ((st = upload(p, t.b_entry, &d.b_entry)) != HEGET_OK) return st;
-    if ((st = upload(p, t.b_vtab, &d.b_vtab)) != HEGET_OK) return st;
-    if ((st = upload(p, t.jl_index, &d.jl_index)) != HEGET_OK) return st;
-    if ((st = upload(p, t.jl_coef, &d.jl_coef)) != HEGET_OK) return st;
+    {   // closing records in the byte layout of this precision (heget_tab.cuh, tab_load_ops / tab_finish)
+        const bool f64 = p->prec == HEGET_FP64;
+        const unsigned scale = f64 ? 2u : 1u, esz = f64 ? 8u : 4u;
+        const size_t ENT = f64 ? hg::tab_entry_bytes<double>() : hg::tab_entry_bytes<float>(), LT = (size_t)t.nchunks * 32;
+        const size_t npad = (size_t)t.n_entries + HG_TAB_RING + 2;
+        std::vector<unsigned char> ent(npad * ENT, 0);
+        for (size_t k = 0; k < npad; ++k) {
+            uint32_t w[28]; memset(w, 0, sizeof w);
+            if (k >= (size_t)t.n_entries) { w[0] = 3u; memcpy(&ent[k * ENT], w, ENT); continue; }      // null record: no amplitude, no update
+            const uint32_t* e = &t.b_rec[k * 16];
+            const unsigned kind = e[0] & 3u, reset = (e[0] >> 2) & 1u, nu = (e[0] >> 3) & 7u;
+            const unsigned base[4] = {e[1] & 0xffffu, e[1] >> 16, e[2] & 0xffffu, e[2] >> 16};
+            unsigned row[4], stride[4];
+            for (int j = 0; j < 4; ++j) { row[j] = ((e[3] >> (8 * j)) & 0xffu) * (unsigned)LT; stride[j] = 1u << ((e[0] >> (8 + 3 * j)) & 7u); if (scale * base[j] > 0xffffu || row[j] > 0xffffu) return fail(HEGET_EUNSUPPORTED, "process '%s': current store too large for the table format", p->name.c_str()); }
+            const unsigned frow = (e[4] & 0xffu) * (unsigned)LT, ka = ((e[4] >> 8) & 0xffu) * 4u * esz, kb = ((e[4] >> 16) & 0xffu) * 4u * esz;
+            if (frow > 0xffffu || ka > 0xffffu || kb > 0xffffu) return fail(HEGET_EUNSUPPORTED, "process '%s': tables too large for the record format", p->name.c_str());
+            w[0] = kind | (reset << 2) | (nu << 3) | (frow << 16);
+            w[1] = scale * base[0] | (scale * base[1] << 16); w[2] = scale * base[2] | (scale * base[3] << 16);
+            w[3] = row[0] | (row[1] << 16); w[4] = row[2] | (row[3] << 16);
+            w[5] = stride[0] | (stride[1] << 8) | (stride[2] << 16) | (stride[3] << 24);
+            w[6] = ka | (kb << 16);
+            const double sgn = t.coef[e[5]];
+            if (f64) {
+                memcpy(&w[8], &sgn, 8);
+                for (unsigned j = 0; j < nu; ++j) { const double c = t.coef[e[6 + j] >> 16]; w[12 + 4 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 8u; memcpy(&w[14 + 4 * j], &c, 8); }
+            } else {
+                const float sf = (float)sgn; memcpy(&w[7], &sf, 4);
+                for (unsigned j = 0; j < nu; ++j) { const float c = (float)t.coef[e[6 + j] >> 16]; w[8 + 2 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 4u; memcpy(&w[9 + 2 * j], &c, 4); }
+            }
+            memcpy(&ent[k * ENT], w, ENT);
+        }
+        if ((st = upload(p, ent, &d.b_ent)) != HEGET_OK) return st;
+        std::vector<unsigned char> rows(t.lanerows.begin(), t.lanerows.end()); rows.resize((rows.size() + 15) / 16 * 16 + 16, 0);
+        if ((st = upload(p, rows, &d.lanerows)) != HEGET_OK) return st;
+        d.n_entries = t.n_entries; d.n_rows = t.n_rows;
+    }
     if ((st = upload(p, t.evalidx, &d.evalidx)) != HEGET_OK) return st;
     if (p->prec == HEGET_FP64) {
         const double* c = 0; if ((st = upload(p, t.cmat, &c)) != HEGET_OK) return st; d.cmat = c;
@@ -243,11 +306,12 @@ static heget_status_t table_to_device(heget_process* p) {
         if ((st = upload(p, cm, &c)) != HEGET_OK) return st; d.cmat = c;
         if ((st = upload(p, cf, &c)) != HEGET_OK) return st; d.coef = c;
     }
-    size_t smem = 0;
-    p->tab_epc = p->prec == HEGET_FP64 ? tab_pick_epc<double>(d, &smem) : tab_pick_epc<float>(d, &smem);
-    if (p->tab_epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
-    if (p->prec == HEGET_FP64) CU(cudaFuncSetAttribute(hg::k_tab<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    else CU(cudaFuncSetAttribute(hg::k_tab<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    p->tab_shape = tab_shape_of(d, p->prec);
+    if (p->tab_shape.epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
+    p->tab_epc = p->tab_shape.epc;
+    const int smem = (int)p->tab_shape.smem;
+    if (p->prec == HEGET_FP64) { if (p->tab_shape.jm) CU(cudaFuncSetAttribute(hg::k_tab<double, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); else CU(cudaFuncSetAttribute(hg::k_tab<double, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); }
+    else { if (p->tab_shape.jm) CU(cudaFuncSetAttribute(hg::k_tab<float, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); else CU(cudaFuncSetAttribute(hg::k_tab<float, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); }
     p->tab_on_device = true;
     return HEGET_OK;
 }
@@ -287,6 +351,7 @@ heget_status_t heget_process_create(const char* process, double sqrt_s_hat, doub
     if (!p) return fail(HEGET_ENOMEM, "out of host memory");
     p->d = 0; p->tab = 0; p->tab_on_device = false; p->tab_epc = 0; p->name = name; p->tag = tag; p->n_legs = n_legs;
     p->kernel_req = prec == HEGET_FP32X2 ? HEGET_KERNEL_STRAIGHT : HEGET_KERNEL_AUTO;
+    { int ng = 0; const std::string padded = " " + name + " "; for (size_t q = 0; q + 2 < padded.size(); ++q) if (padded[q] == ' ' && padded[q + 1] == 'g' && padded[q + 2] == ' ') ++ng; p->auto_table = n_legs >= 7 || (n_legs == 6 && ng >= 6); }
     p->prec = (int)prec; p->lanes = 0; p->sqrt_s = sqrt_s_hat; p->alpha_s = alpha_s;
     p->cuts.pt_min = cuts ? cuts->pt_min : 0.0; p->cuts.eta_max = cuts ? cuts->eta_max : 0.0; p->cuts.dr_min = cuts ? cuts->dr_min : 0.0;
     p->s_mom = 0; p->s_w = 0; p->s_me2 = 0; p->s_cap = 0;
@@ -349,12 +414,15 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
         o->avg_spin = t.avg_spin; o->avg_color = t.avg_color; o->sym_factor = t.sym_factor;
         o->flops_per_event = t.flops_per_event; o->flops_per_helicity = t.flops_per_hel;
         o->lanes_wide = 32; o->lanes = 32;
-        hg::TabDev d; memset(&d, 0, sizeof d); d.n_ext = t.n_ext; d.nchunks = t.nchunks; d.R = t.R; d.nK = t.nK; d.store32 = t.store32;
-        const int epc = p->prec == HEGET_FP64 ? tab_pick_epc<double>(d, 0) : tab_pick_epc<float>(d, 0);
-        o->events_per_block = epc; o->threads_per_block = epc * t.nchunks * 32;
+        hg::TabDev d; memset(&d, 0, sizeof d); d.n_ext = t.n_ext; d.nchunks = t.nchunks; d.R = t.R; d.nK = t.nK; d.store32 = t.store32; d.n_rows = t.n_rows;
+        d.Rpad = t.Rpad;
+        const TabShape sh = tab_shape_of(d, p->prec);
+        o->events_per_block = sh.epc; o->threads_per_block = sh.epc * t.nchunks * 32; o->j_in_tmem = sh.jm;
         if (have_dev) {
             cudaFuncAttributes fa;
-            const cudaError_t e = p->prec == HEGET_FP64 ? cudaFuncGetAttributes(&fa, hg::k_tab<double>) : cudaFuncGetAttributes(&fa, hg::k_tab<float>);
+            cudaError_t e;
+            if (p->prec == HEGET_FP64) e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<double, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<double, 0>);
+            else e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<float, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<float, 0>);
             if (e == cudaSuccess) { o->regs_per_thread = fa.numRegs; o->local_bytes_per_thread = (int)fa.localSizeBytes; } else cudaGetLastError();
         }
         return HEGET_OK;
@@ -447,13 +515,12 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         if (blocks > 0x7fffffffull) return fail(HEGET_EINVAL, "heget_eval_me2: n_events too large for one launch");
         const int threads = epc * p->tdev.nchunks * 32;
         cudaStream_t s = (cudaStream_t)cuda_stream;
-        if (p->prec == HEGET_FP64) {
-            const size_t smem = hg::tab_smem_bytes<double>(p->tdev, epc) + 32;
-            hg::k_tab<double><<<(unsigned int)blocks, threads, smem, s>>>(p->tdev, epc, d_mom, n_events, 1.0 / p->sqrt_s, p->out_scale, (double*)d_me2, (int)mode, hel_fixed, seed, first_event);
-        } else {
-            const size_t smem = hg::tab_smem_bytes<float>(p->tdev, epc) + 32;
-            hg::k_tab<float><<<(unsigned int)blocks, threads, smem, s>>>(p->tdev, epc, d_mom, n_events, 1.0 / p->sqrt_s, p->out_scale, (float*)d_me2, (int)mode, hel_fixed, seed, first_event);
-        }
+        const TabShape& sh = p->tab_shape;
+        const double iss = 1.0 / p->sqrt_s;
+#define HG_TAB_LAUNCH(TT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)blocks, threads, sh.smem, s>>>(p->tdev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, iss, p->out_scale, (TT*)d_me2, (int)mode, hel_fixed, seed, first_event)
+        if (p->prec == HEGET_FP64) { if (sh.jm) HG_TAB_LAUNCH(double, 1); else HG_TAB_LAUNCH(double, 0); }
+        else { if (sh.jm) HG_TAB_LAUNCH(float, 1); else HG_TAB_LAUNCH(float, 0); }
+#undef HG_TAB_LAUNCH
         CU(cudaGetLastError());
         g_launches++;
         return HEGET_OK;

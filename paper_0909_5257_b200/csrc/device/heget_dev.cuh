@@ -122,7 +122,13 @@ template <typename T> HG_HD T mdot(const mom4<T>& a, const mom4<T>& b) { return 
 
 // Minkowski products (bilinear, no complex conjugation)
 template <typename T> HG_HD cx<T> vdot(const vec4<T>& a, const vec4<T>& b) {
-    return a.v[0] * b.v[0] - a.v[1] * b.v[1] - a.v[2] * b.v[2] - a.v[3] * b.v[3];
+    // one expression per component: every product after the first contracts into an FMA (2 MUL + 14 FMA instead of 8 + 8 + 6 ADD)
+    cx<T> r;
+    r.re = a.v[0].re * b.v[0].re - a.v[0].im * b.v[0].im - a.v[1].re * b.v[1].re + a.v[1].im * b.v[1].im
+         - a.v[2].re * b.v[2].re + a.v[2].im * b.v[2].im - a.v[3].re * b.v[3].re + a.v[3].im * b.v[3].im;
+    r.im = a.v[0].re * b.v[0].im + a.v[0].im * b.v[0].re - a.v[1].re * b.v[1].im - a.v[1].im * b.v[1].re
+         - a.v[2].re * b.v[2].im - a.v[2].im * b.v[2].re - a.v[3].re * b.v[3].im - a.v[3].im * b.v[3].re;
+    return r;
 }
 template <typename T> HG_HD cx<T> kdot(const mom4<T>& k, const vec4<T>& a) {
     return mk<T>(k.p[0] * a.v[0].re - k.p[1] * a.v[1].re - k.p[2] * a.v[2].re - k.p[3] * a.v[3].re,

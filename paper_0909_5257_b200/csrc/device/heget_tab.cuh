@@ -22,6 +22,7 @@
 // the same chunk (multicast), lanes with different variants read neighbouring chunks (no bank conflict).
 #pragma once
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
 #include "heget_dev.cuh"
 #include "heget_rt.cuh"
@@ -32,8 +33,9 @@ struct TabDev {
     int n_ext, NH, nchunks, cpc, R, Rpad, nK, store32, n_levels, n_closings;
     const uint32_t* kmask; const uint32_t* leginfo;
     const uint32_t* a_hdr; const uint32_t* a_out; const uint32_t* a_term; const uint32_t* a_level;
-    const uint32_t* b_entry; const uint32_t* b_vtab;
-    const uint16_t* jl_index; const uint16_t* jl_coef;
+    int n_entries, n_rows;
+    const unsigned char* b_ent;  // [n_entries + padding] closing records in the byte layout of this precision (tab_entry_bytes<T>() each; api.cu, table_to_device)
+    const unsigned char* lanerows; // [n_rows][nchunks * 32] per-lane bytes: variant of a leg set, or validity | chirality << 1
     const void* coef;            // T[]: pool of rational coefficients
     const void* cmat;            // T[(Rpad/8) * R * 8]
     const short* evalidx;        // [2^n_ext] helicity bits -> evaluated configuration or -1
@@ -44,8 +46,13 @@ template <typename T> __host__ __device__ inline size_t tab_event_bytes(int nK, 
     return (size_t)nK * 4 * sizeof(T) + (((size_t)nK * sizeof(T) + 15) / 16) * 16 + (size_t)store32 * 16 * (sizeof(T) / 4);
 }
 template <typename T> __host__ __device__ inline size_t tab_warp_bytes(int R) { return (size_t)2 * R * 32 * sizeof(T); }
-template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc) {
-    return (size_t)epc * (sizeof(double) * 4 * d.n_ext + tab_event_bytes<T>(d.nK, d.store32) + (size_t)d.nchunks * tab_warp_bytes<T>(d.R) + sizeof(double) * d.nchunks);
+// a closing record is 64 bytes in FP32 (16 words) and 112 bytes in FP64; every warp keeps TAB_RING of them in flight
+template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { return sizeof(T) == 4 ? 64 : 112; }
+#define HG_TAB_RING 8
+template <typename T> __host__ __device__ inline size_t tab_rows_bytes(int n_rows, int nchunks) { return (((size_t)n_rows * nchunks * 32) + 15) / 16 * 16; }
+template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, bool j_in_tmem = false) {
+    return (size_t)epc * (sizeof(double) * 4 * d.n_ext + tab_event_bytes<T>(d.nK, d.store32) + (size_t)d.nchunks * ((j_in_tmem ? 0 : tab_warp_bytes<T>(d.R)) + HG_TAB_RING * tab_entry_bytes<T>()) + sizeof(double) * d.nchunks)
+           + tab_rows_bytes<T>(d.n_rows, d.nchunks);
 }
 
 #if defined(__CUDACC__)
@@ -110,8 +117,200 @@ template <typename T> __device__ __forceinline__ void sacc(sp2<T>& a, const sp2<
     a.s[0].re += b.s[0].re; a.s[0].im += b.s[0].im; a.s[1].re += b.s[1].re; a.s[1].im += b.s[1].im;
 }
 
-template <typename T>
-__global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, const double* __restrict__ mom, const unsigned long long n_events,
+
+// ---- phase B helpers ------------------------------------------------------------------------------------------------------
+// operands of one closing in registers: VVV w[0..3] = a, w[4..7] = b, w[8..11] = c, k = (ka, kb, kc); GGGG w[0..15] = a, b, c, d;
+// IOV w[0..1] = psi, w[2..3] = psibar, w[4..7] = gluon
+template <typename T> struct TabOps { cx<T> w[16]; T k[12]; };
+
+template <typename T> __device__ __forceinline__ void tab_ld(cx<T>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp);
+template <> __device__ __forceinline__ void tab_ld<float>(cx<float>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp) {
+    const float4* s = reinterpret_cast<const float4*>(store) + addr;
+    const float4 c0 = s[0]; w[0] = mk<float>(c0.x, c0.y); w[1] = mk<float>(c0.z, c0.w);
+    if (ncomp == 4) { const float4 c1 = s[stride]; w[2] = mk<float>(c1.x, c1.y); w[3] = mk<float>(c1.z, c1.w); }
+}
+template <> __device__ __forceinline__ void tab_ld<double>(cx<double>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp) {
+    const double2* s = reinterpret_cast<const double2*>(store) + addr;
+    const double2 c0 = s[0], c1 = s[stride]; w[0] = mk<double>(c0.x, c0.y); w[1] = mk<double>(c1.x, c1.y);
+    if (ncomp == 4) { const double2 c2 = s[2 * stride], c3 = s[3 * stride]; w[2] = mk<double>(c2.x, c2.y); w[3] = mk<double>(c3.x, c3.y); }
+}
+template <typename T> __device__ __forceinline__ void tab_ldk4(T* k, const T* p);
+template <> __device__ __forceinline__ void tab_ldk4<float>(float* k, const float* p) { const float4 c = *reinterpret_cast<const float4*>(p); k[0] = c.x; k[1] = c.y; k[2] = c.z; k[3] = c.w; }
+template <> __device__ __forceinline__ void tab_ldk4<double>(double* k, const double* p) { const double2 c0 = reinterpret_cast<const double2*>(p)[0], c1 = reinterpret_cast<const double2*>(p)[1]; k[0] = c0.x; k[1] = c0.y; k[2] = c1.x; k[3] = c1.y; }
+// closing record (uniform, in the warp's ring).  Word 0: kind (0 vvv, 1 gggg, 2 iov, 3 updates only) | reset S << 2 | updates << 3 |
+// byte offset of the flag row << 16; words 1-2: chunk bases of the operands a | b << 16, c | d << 16; words 3-4: byte offsets of their
+// variant rows; word 5: strides (chunks between the 16-byte pieces of one variant) a | b << 8 | c << 16 | d << 24; word 6: byte offsets
+// of K_a | K_b << 16 in the momentum slots; FP32: word 7 = group coefficient, words 8-15 = 4 x {byte offset of Re J_k, coefficient};
+// FP64: words 8-9 = group coefficient, words 12-27 = 4 x {offset, 0, coefficient}
+template <typename T> struct TabCtl { unsigned ctl; T sg; bool chi; };
+
+template <typename T> __device__ __forceinline__ void tab_load_ops(TabOps<T>& O, TabCtl<T>& C, const unsigned char* ent, const unsigned char* store, const T* evK, const unsigned char* myrows) {
+    const uint4 q0 = *reinterpret_cast<const uint4*>(ent), q1 = *reinterpret_cast<const uint4*>(ent + 16);
+    const unsigned kind = q0.x & 3u;
+    C.ctl = q0.x;
+    T sgc;
+    if constexpr (sizeof(T) == 4) sgc = __uint_as_float(q1.w); else sgc = *reinterpret_cast<const double*>(ent + 32);
+    const unsigned fb = myrows[q0.x >> 16];
+    C.sg = (fb & 1u) ? sgc : T(0); C.chi = (fb & 2u) != 0u;
+    if (kind == 3u) return;
+    const unsigned aa = (q0.y & 0xffffu) + myrows[q0.w & 0xffffu], ab = (q0.y >> 16) + myrows[q0.w >> 16], ac = (q0.z & 0xffffu) + myrows[q1.x & 0xffffu];
+    const unsigned sa = q1.y & 0xffu, sb = (q1.y >> 8) & 0xffu, sc = (q1.y >> 16) & 0xffu;
+    if (kind == 0u) {
+        tab_ld<T>(O.w, store, aa, sa, 4); tab_ld<T>(O.w + 4, store, ab, sb, 4); tab_ld<T>(O.w + 8, store, ac, sc, 4);
+        const T* ka = reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(evK) + (q1.z & 0xffffu));
+        const T* kb = reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(evK) + (q1.z >> 16));
+        tab_ldk4<T>(O.k, ka); tab_ldk4<T>(O.k + 4, kb);
+    } else if (kind == 1u) {
+        const unsigned ad = (q0.z >> 16) + myrows[q1.x >> 16], sd = q1.y >> 24;
+        tab_ld<T>(O.w, store, aa, sa, 4); tab_ld<T>(O.w + 4, store, ab, sb, 4); tab_ld<T>(O.w + 8, store, ac, sc, 4); tab_ld<T>(O.w + 12, store, ad, sd, 4);
+    } else {
+        tab_ld<T>(O.w, store, aa, sa, 2); tab_ld<T>(O.w + 2, store, ab, sb, 2); tab_ld<T>(O.w + 4, store, ac, sc, 4);
+    }
+}
+template <typename T> __device__ __forceinline__ cx<T> tab_dot(const cx<T>* a, const cx<T>* b) {      // Minkowski product, 2 MUL + 14 FMA
+    cx<T> r;
+    r.re = a[0].re * b[0].re - a[0].im * b[0].im - a[1].re * b[1].re + a[1].im * b[1].im - a[2].re * b[2].re + a[2].im * b[2].im - a[3].re * b[3].re + a[3].im * b[3].im;
+    r.im = a[0].re * b[0].im + a[0].im * b[0].re - a[1].re * b[1].im - a[1].im * b[1].re - a[2].re * b[2].im - a[2].im * b[2].re - a[3].re * b[3].im - a[3].im * b[3].re;
+    return r;
+}
+template <typename T> __device__ __forceinline__ cx<T> tab_kdot(const T* k1, const T* k2, const cx<T>* a) {       // (k1 - k2) . a
+    const T d0 = k1[0] - k2[0], d1 = k1[1] - k2[1], d2 = k1[2] - k2[2], d3 = k1[3] - k2[3];
+    return mk<T>(d0 * a[0].re - d1 * a[1].re - d2 * a[2].re - d3 * a[3].re, d0 * a[0].im - d1 * a[1].im - d2 * a[2].im - d3 * a[3].im);
+}
+template <typename T> __device__ __forceinline__ cx<T> tab_kvec(const T* d, const cx<T>* a) {
+    return mk<T>(d[0] * a[0].re - d[1] * a[1].re - d[2] * a[2].re - d[3] * a[3].re, d[0] * a[0].im - d[1] * a[1].im - d[2] * a[2].im - d[3] * a[3].im);
+}
+// vvvxxx (eq. 24-27) with unit coupling: (a.b)((ka-kb).c) + (b.c)((kb-kc).a) + (c.a)((kc-ka).b)
+template <typename T> __device__ __forceinline__ cx<T> tab_vvv(const TabOps<T>& O) {
+    const cx<T>* a = O.w; const cx<T>* b = O.w + 4; const cx<T>* c = O.w + 8;
+    const cx<T> ab = tab_dot<T>(a, b), bc = tab_dot<T>(b, c), ca = tab_dot<T>(c, a);
+    // all momenta flow into the vertex, ka + kb + kc = 0:  kb - kc = ka + 2 kb,  kc - ka = -(2 ka + kb)
+    T kbc[4], kca[4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { kbc[m] = O.k[m] + T(2) * O.k[4 + m]; kca[m] = -(T(2) * O.k[m] + O.k[4 + m]); }
+    const cx<T> x = tab_kdot<T>(O.k, O.k + 4, c), y = tab_kvec<T>(kbc, a), z = tab_kvec<T>(kca, b);
+    return mk<T>(ab.re * x.re - ab.im * x.im + bc.re * y.re - bc.im * y.im + ca.re * z.re - ca.im * z.im,
+                 ab.re * x.im + ab.im * x.re + bc.re * y.im + bc.im * y.re + ca.re * z.im + ca.im * z.re);
+}
+// ggggxx (eqs. 32-36) with unit coupling, the piece being encoded in the operand order: (a.d)(b.c) - (a.c)(b.d)
+template <typename T> __device__ __forceinline__ cx<T> tab_gggg(const TabOps<T>& O) {
+    const cx<T>* a = O.w; const cx<T>* b = O.w + 4; const cx<T>* c = O.w + 8; const cx<T>* dd = O.w + 12;
+    const cx<T> p = tab_dot<T>(a, dd), q = tab_dot<T>(b, c), r = tab_dot<T>(a, c), s = tab_dot<T>(b, dd);
+    return mk<T>(p.re * q.re - p.im * q.im - r.re * s.re + r.im * s.im, p.re * q.im + p.im * q.re - r.re * s.im - r.im * s.re);
+}
+// iovxx0 (eqs. 18-22) with unit coupling
+template <typename T> __device__ __forceinline__ cx<T> tab_iov(const TabOps<T>& O, T chi) {
+    sp2<T> fi, fo; vec4<T> vc;
+    fi.s[0] = O.w[0]; fi.s[1] = O.w[1]; fo.s[0] = O.w[2]; fo.s[1] = O.w[3];
+    vc.v[0] = O.w[4]; vc.v[1] = O.w[5]; vc.v[2] = O.w[6]; vc.v[3] = O.w[7];
+    return iovxx0<T>(fi, fo, vc, chi, T(1));
+}
+
+// ---- where a warp keeps its block of J (R complex numbers per lane) -----------------------------------------------------------
+// JSmem: shared memory, element (k, re/im) of lane l at J[(2k + ri) * 32 + l].
+// JTmem: tensor memory (TMEM, 256 kB per SM beside the 228 kB of shared memory): lane l of the warp's 32-lane quadrant, columns
+//        2k, 2k+1 (FP32) or 4k..4k+3 (FP64), moved with tcgen05.ld / tcgen05.st (SASS: LDTM / STTM).  J is the largest per-warp
+//        buffer (30 kB in FP32, 61 kB in FP64 for 120 colour elements): in TMEM it costs no shared memory, so twice as many warps
+//        are resident for the processes whose J limited the occupancy, and its read-modify-write traffic leaves the LSU pipe.
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void tm_ld2(unsigned ta, unsigned& a, unsigned& b) { asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];\n" : "=r"(a), "=r"(b) : "r"(ta)); }
+__device__ __forceinline__ void tm_ld4(unsigned ta, unsigned& a, unsigned& b, unsigned& c, unsigned& d) { asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];\n" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(ta)); }
+__device__ __forceinline__ void tm_st2(unsigned ta, unsigned a, unsigned b) { asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};\n" :: "r"(ta), "r"(a), "r"(b) : "memory"); }
+__device__ __forceinline__ void tm_st4(unsigned ta, unsigned a, unsigned b, unsigned c, unsigned d) { asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};\n" :: "r"(ta), "r"(a), "r"(b), "r"(c), "r"(d) : "memory"); }
+
+template <typename T> struct JSmem {
+    T* J;
+    __device__ __forceinline__ void zero(int R) { for (int a = 0; a < 2 * R; ++a) J[a * 32] = T(0); }
+    // J_k += c_j (Sr, Si) for the nu <= 4 updates of a record; off = byte offset of Re J_k in the lane's column
+    __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (j < nu) { T* pj = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(J) + off[j]); pj[0] += c[j] * Sr; pj[32] += c[j] * Si; }
+    }
+    // 8 consecutive elements starting at k0 (k0 a multiple of 8)
+    __device__ __forceinline__ void block8(int k0, int R, T* xr, T* xi) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { const bool in = k0 + i < R; xr[i] = in ? J[(2 * (k0 + i)) * 32] : T(0); xi[i] = in ? J[(2 * (k0 + i) + 1) * 32] : T(0); }
+    }
+};
+template <typename T> struct JTmem;
+template <> struct JTmem<float> {
+    unsigned ta;      // TMEM address of column 0 of this warp's block (lane field = first lane of the warp's quadrant)
+    __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st2(ta + 2 * k, 0u, 0u); tm_wait_st(); }
+    __device__ __forceinline__ void update(int nu, const unsigned* off, const float* c, float Sr, float Si) {
+        unsigned r[4][2];
+        tm_wait_st();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (j < nu) tm_ld2(ta + (off[j] >> 7), r[j][0], r[j][1]);
+        tm_wait_ld();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (j < nu) tm_st2(ta + (off[j] >> 7), __float_as_uint(__uint_as_float(r[j][0]) + c[j] * Sr), __float_as_uint(__uint_as_float(r[j][1]) + c[j] * Si));
+    }
+    __device__ __forceinline__ void block8(int k0, int, float* xr, float* xi) {
+        unsigned r[8][2];
+        tm_wait_st();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) tm_ld2(ta + 2 * (k0 + i), r[i][0], r[i][1]);
+        tm_wait_ld();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { xr[i] = __uint_as_float(r[i][0]); xi[i] = __uint_as_float(r[i][1]); }
+    }
+};
+template <> struct JTmem<double> {
+    unsigned ta;
+    __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st4(ta + 4 * k, 0u, 0u, 0u, 0u); tm_wait_st(); }
+    __device__ __forceinline__ void update(int nu, const unsigned* off, const double* c, double Sr, double Si) {
+        unsigned r[4][4];
+        tm_wait_st();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (j < nu) tm_ld4(ta + (off[j] >> 7), r[j][0], r[j][1], r[j][2], r[j][3]);
+        tm_wait_ld();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (j < nu) {
+            const double re = __hiloint2double((int)r[j][1], (int)r[j][0]) + c[j] * Sr, im = __hiloint2double((int)r[j][3], (int)r[j][2]) + c[j] * Si;
+            tm_st4(ta + (off[j] >> 7), (unsigned)__double2loint(re), (unsigned)__double2hiint(re), (unsigned)__double2loint(im), (unsigned)__double2hiint(im));
+        }
+    }
+    __device__ __forceinline__ void block8(int k0, int, double* xr, double* xi) {
+        unsigned r[8][4];
+        tm_wait_st();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) tm_ld4(ta + 4 * (k0 + i), r[i][0], r[i][1], r[i][2], r[i][3]);
+        tm_wait_ld();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { xr[i] = __hiloint2double((int)r[i][1], (int)r[i][0]); xi[i] = __hiloint2double((int)r[i][3], (int)r[i][2]); }
+    }
+};
+
+// amplitude of one closing into its group sum; at the end of a group, J_k += x_gk S_g (eq. 8) on the lane's column
+template <typename T, typename JP> __device__ __forceinline__ void tab_finish(const TabOps<T>& O, const TabCtl<T>& C, const unsigned char* ent, JP& jp, T& Sr, T& Si) {
+    const unsigned kind = C.ctl & 3u;
+    if (kind != 3u) {
+        cx<T> amp;
+        if (kind == 0u) amp = tab_vvv<T>(O);
+        else if (kind == 1u) amp = tab_gggg<T>(O);
+        else amp = tab_iov<T>(O, C.chi ? T(1) : T(-1));
+        Sr += C.sg * amp.re; Si += C.sg * amp.im;
+    }
+    const int nu = (C.ctl >> 3) & 7u;
+    if (nu) {
+        unsigned off[4]; T c[4];
+        if constexpr (sizeof(T) == 4) {
+            const uint4 u0 = *reinterpret_cast<const uint4*>(ent + 32), u1 = *reinterpret_cast<const uint4*>(ent + 48);
+            off[0] = u0.x; c[0] = __uint_as_float(u0.y); off[1] = u0.z; c[1] = __uint_as_float(u0.w);
+            off[2] = u1.x; c[2] = __uint_as_float(u1.y); off[3] = u1.z; c[3] = __uint_as_float(u1.w);
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { const uint4 uu = *reinterpret_cast<const uint4*>(ent + 48 + 16 * j); off[j] = uu.x; c[j] = __hiloint2double((int)uu.w, (int)uu.z); }
+        }
+        jp.update(nu, off, c, Sr, Si);
+    }
+    if (C.ctl & 4u) { Sr = T(0); Si = T(0); }
+}
+
+// JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp)
+template <typename T, int JM>
+__global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long n_events,
         const double inv_sqrt_s, const double out_scale, T* __restrict__ me2, const int hel_mode, const int hel_fixed,
         const unsigned long long seed, const unsigned long long first_event) {
     typedef tabio<T> IO;
@@ -128,7 +327,23 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     T* evK = reinterpret_cast<T*>(myev);
     T* evI = evK + (size_t)4 * d.nK;
     unsigned char* store = myev + (size_t)d.nK * 4 * sizeof(T) + (((size_t)d.nK * sizeof(T) + 15) / 16) * 16;
-    T* J = reinterpret_cast<T*>(evbase + (size_t)epc * evb + (size_t)(el * wpe + wie) * tab_warp_bytes<T>(d.R)) + lane;
+    unsigned char* jbase = evbase + (size_t)epc * evb;
+    const size_t jwb = JM ? 0 : tab_warp_bytes<T>(d.R);
+    typename std::conditional<JM == 0, JSmem<T>, JTmem<T> >::type jp;
+    if constexpr (JM == 0) jp.J = reinterpret_cast<T*>(jbase + (size_t)(el * wpe + wie) * jwb) + lane;
+    unsigned char* ring = jbase + (size_t)epc * wpe * jwb + (size_t)(el * wpe + wie) * (HG_TAB_RING * tab_entry_bytes<T>());
+    unsigned char* rows = jbase + (size_t)epc * wpe * (jwb + HG_TAB_RING * tab_entry_bytes<T>());
+    __shared__ unsigned int tm_base;
+    if constexpr (JM == 1) {
+        // one warp allocates the CTA's TMEM columns and gives up the permit at once, so co-resident CTAs can allocate theirs
+        if (tid < 32) {
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&tm_base);
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" :: "r"(dst), "r"((unsigned)tm_cols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+    }
+    for (int c = tid; c < (d.n_rows * wpe * 32 + 3) / 4; c += blockDim.x) reinterpret_cast<unsigned int*>(rows)[c] = __ldg(reinterpret_cast<const unsigned int*>(d.lanerows) + c);
 
     const unsigned long long e0 = (unsigned long long)blockIdx.x * epc;
     unsigned long long e = e0 + el;
@@ -142,6 +357,11 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
         pm[c] = mom[(size_t)(c / epc) * n_events + ee] * inv_sqrt_s;
     }
     __syncthreads();
+    if constexpr (JM == 1) {
+        asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+        const int wic = tid >> 5;       // warp w of the CTA owns TMEM lanes 32 (w % 4) .. +31, and the (w / 4)-th block of tm_wcols columns
+        jp.ta = tm_base + ((unsigned)((wic & 3) * 32) << 16) + (unsigned)((wic >> 2) * tm_wcols);
+    }
     {
         const double* pe = pm + el;
         for (int s = te; s < d.nK; s += tpe) {       // momentum of a leg subset, all momenta flowing INTO the diagram, and 1/q^2
@@ -232,71 +452,85 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     T form = T(0);
     if (chunk_on) {
         const int R = d.R;
-        for (int a = 0; a < 2 * R; ++a) J[a * 32] = T(0);
+        jp.zero(R);
         T Sr = T(0), Si = T(0);
-        const uint32_t* vt = d.b_vtab + (size_t)wie * 32 + lane;
-        const int stride = wpe * 32;
-        for (int k = 0; k < d.n_closings; ++k) {
-            const uint4 e0w = __ldg(reinterpret_cast<const uint4*>(d.b_entry) + 2 * k);
-            const uint2 e1w = __ldg(reinterpret_cast<const uint2*>(d.b_entry) + 4 * k + 2);
-            const unsigned w = __ldg(vt + (size_t)k * stride);
-            const unsigned ba = e0w.x & 0xffffu, bb = e0w.x >> 16, bc = e0w.y & 0xffffu, bd = e0w.y >> 16;
-            const unsigned la = e0w.z & 7u, lb = (e0w.z >> 3) & 7u, lc = (e0w.z >> 6) & 7u, ld = (e0w.z >> 9) & 7u, kind = (e0w.z >> 12) & 7u;
-            const unsigned va = w & 31u, vb = (w >> 5) & 31u, vc = (w >> 10) & 31u, vd = (w >> 15) & 31u;
-            cx<T> amp;
-            if (kind == 0u) {
-                amp = vvvxxx<T>(IO::ldv(store, ba + va, la), IO::ldk(evK, (e0w.z >> 16) & 0xffu), IO::ldv(store, bb + vb, lb), IO::ldk(evK, e0w.z >> 24),
-                                IO::ldv(store, bc + vc, lc), IO::ldk(evK, e0w.w & 0xffu), T(1));
-            } else if (kind == 1u) {
-                amp = ggggxx<T>(IO::ldv(store, ba + va, la), IO::ldv(store, bb + vb, lb), IO::ldv(store, bc + vc, lc), IO::ldv(store, bd + vd, ld), T(1));
-            } else {
-                const T chi = ((w >> 20) & 1u) ? T(1) : T(-1);
-                amp = iovxx0<T>(IO::lds(store, ba + va, la), IO::lds(store, bb + vb, lb), IO::ldv(store, bc + vc, lc), chi, T(1));
+        constexpr int ENT = tab_entry_bytes<T>(), NS = HG_TAB_RING;
+        const unsigned char* gent = d.b_ent;
+        const unsigned char* myrows = rows + wie * 32 + lane;
+        // the closing records stream through a per-warp ring in shared memory, NS - 1 records ahead of their use (cp.async),
+        // so the table latency (L2) never shows; operands are fetched one closing ahead of the arithmetic, and the loop is
+        // unrolled by two so that the two operand sets alternate without register copies
+        auto issue = [&](int k) {
+            if (lane < ENT / 16) {
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + (k & (NS - 1)) * ENT + lane * 16);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst), "l"(gent + (size_t)k * ENT + lane * 16));
             }
-            const T sg = ((w >> 21) & 1u) ? __ldg(cf + e1w.x) : T(0);
-            Sr += sg * amp.re; Si += sg * amp.im;
-            if ((e0w.z >> 15) & 1u) {
-                const int jc = (e0w.w >> 8) & 0xff; const unsigned jo = e1w.y;
-                for (int j = 0; j < jc; ++j) {
-                    const int idx = __ldg(d.jl_index + jo + j); const T c = __ldg(cf + __ldg(d.jl_coef + jo + j));
-                    J[(2 * idx) * 32] += c * Sr; J[(2 * idx + 1) * 32] += c * Si;
-                }
-                Sr = T(0); Si = T(0);
-            }
+            asm volatile("cp.async.commit_group;\n" ::);
+        };
+        auto landed = [&]() { asm volatile("cp.async.wait_group %0;\n" :: "n"(NS - 2)); __syncwarp(); };
+        const int nent = d.n_entries;
+        for (int k = 0; k < NS - 1; ++k) issue(k);           // the table is padded with NS + 2 null records
+        landed();
+        TabOps<T> O0, O1;
+        TabCtl<T> C0, C1;
+        tab_load_ops<T>(O0, C0, ring, store, evK, myrows);
+        for (int k = 0; k < nent; k += 2) {
+            issue(k + NS - 1); landed();
+            tab_load_ops<T>(O1, C1, ring + ((k + 1) & (NS - 1)) * ENT, store, evK, myrows);
+            tab_finish<T>(O0, C0, ring + (k & (NS - 1)) * ENT, jp, Sr, Si);
+            issue(k + NS); landed();
+            tab_load_ops<T>(O0, C0, ring + ((k + 2) & (NS - 1)) * ENT, store, evK, myrows);
+            if (k + 1 < nent) tab_finish<T>(O1, C1, ring + ((k + 1) & (NS - 1)) * ENT, jp, Sr, Si);
         }
+        asm volatile("cp.async.wait_all;\n" ::);
         // ---- phase C: colour form on the accumulated basis ----------------------------------------------------------------
         const T* cm = reinterpret_cast<const T*>(d.cmat);
         for (int t = 0; t < d.Rpad / 8; ++t) {
-            T tr[8], ti[8];
+            T tr[8], ti[8], dr[8], di[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) { tr[i] = T(0); ti[i] = T(0); }
             const T* row = cm + (size_t)t * R * 8;
-            for (int b = 8 * t; b < R; ++b) {
-                const T xr = J[(2 * b) * 32], xi = J[(2 * b + 1) * 32];
-                T c8[8];
-                if constexpr (sizeof(T) == 4) {
-                    const float4 c0 = __ldg(reinterpret_cast<const float4*>(row + (size_t)b * 8)), c1 = __ldg(reinterpret_cast<const float4*>(row + (size_t)b * 8) + 1);
-                    c8[0] = c0.x; c8[1] = c0.y; c8[2] = c0.z; c8[3] = c0.w; c8[4] = c1.x; c8[5] = c1.y; c8[6] = c1.z; c8[7] = c1.w;
-                } else {
-                    const double2* rp = reinterpret_cast<const double2*>(row + (size_t)b * 8);
-                    const double2 c0 = __ldg(rp), c1 = __ldg(rp + 1), c2 = __ldg(rp + 2), c3 = __ldg(rp + 3);
-                    c8[0] = c0.x; c8[1] = c0.y; c8[2] = c1.x; c8[3] = c1.y; c8[4] = c2.x; c8[5] = c2.y; c8[6] = c3.x; c8[7] = c3.y;
+            for (int bb = t; bb < d.Rpad / 8; ++bb) {
+                T xr[8], xi[8];
+                jp.block8(8 * bb, R, xr, xi);
+                if (bb == t) {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) { dr[i] = xr[i]; di[i] = xi[i]; }
                 }
 #pragma unroll
-                for (int i = 0; i < 8; ++i) { tr[i] += c8[i] * xr; ti[i] += c8[i] * xi; }
+                for (int q = 0; q < 8; ++q) {
+                    const int b = 8 * bb + q;
+                    if (b < R) {
+                        T c8[8];
+                        if constexpr (sizeof(T) == 4) {
+                            const float4 c0 = __ldg(reinterpret_cast<const float4*>(row + (size_t)b * 8)), c1 = __ldg(reinterpret_cast<const float4*>(row + (size_t)b * 8) + 1);
+                            c8[0] = c0.x; c8[1] = c0.y; c8[2] = c0.z; c8[3] = c0.w; c8[4] = c1.x; c8[5] = c1.y; c8[6] = c1.z; c8[7] = c1.w;
+                        } else {
+                            const double2* rp = reinterpret_cast<const double2*>(row + (size_t)b * 8);
+                            const double2 c0 = __ldg(rp), c1 = __ldg(rp + 1), c2 = __ldg(rp + 2), c3 = __ldg(rp + 3);
+                            c8[0] = c0.x; c8[1] = c0.y; c8[2] = c1.x; c8[3] = c1.y; c8[4] = c2.x; c8[5] = c2.y; c8[6] = c3.x; c8[7] = c3.y;
+                        }
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) { tr[i] += c8[i] * xr[q]; ti[i] += c8[i] * xi[q]; }
+                    }
+                }
             }
 #pragma unroll
-            for (int i = 0; i < 8; ++i) if (8 * t + i < R) form += J[(2 * (8 * t + i)) * 32] * tr[i] + J[(2 * (8 * t + i) + 1) * 32] * ti[i];
+            for (int i = 0; i < 8; ++i) form += dr[i] * tr[i] + di[i] * ti[i];
         }
     }
     // ---- helicity sum (eq. 12) and averaging factors -------------------------------------------------------------
-    double acc = (double)(wgt * form);
+    T acc = wgt * form;          // the helicity sum stays in the kernel's own precision (reading A21)
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) red[el * wpe + wie] = acc;
+    if (lane == 0) red[el * wpe + wie] = (double)acc;
+    if constexpr (JM == 1) { tm_wait_ld(); tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
     __syncthreads();
     if (te == 0 && live) {
-        double s = 0; for (int w = 0; w < wpe; ++w) s += red[el * wpe + w];
-        me2[e] = (T)(out_scale * s);
+        T s = T(0); for (int w = 0; w < wpe; ++w) s += (T)red[el * wpe + w];
+        me2[e] = (T)(out_scale * (double)s);
+    }
+    if constexpr (JM == 1) {
+        if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tm_base), "r"((unsigned)tm_cols) : "memory");
     }
 }
 #endif

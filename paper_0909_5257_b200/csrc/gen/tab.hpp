@@ -284,7 +284,39 @@ struct TabBuilder {
         std::vector<unsigned> cfgbits(P.NH, 0);
         P.hel_table.assign((size_t)P.NH * n, 0); P.evalidx.assign((size_t)1 << n, -1);
         for (int h = 0; h < P.NH; ++h) { std::vector<int> hv = E.hel_of(h); for (int i = 0; i < n; ++i) { P.hel_table[(size_t)h * n + i] = (int8_t)hv[i]; if (hv[i] > 0) cfgbits[h] |= 1u << i; } P.evalidx[cfgbits[h]] = (int16_t)h; }
+        // per-lane byte rows (one byte per helicity configuration of every warp): row of a leg set = the variant index the
+        // configuration selects in a current over those legs; row of (quark-line pairing, line) = bit 0: the configuration
+        // conserves chirality along the closing's quark lines, bit 1: chirality of the closing's own line
+        std::map<unsigned, int> vrow; std::map<std::pair<std::vector<std::pair<int, int> >, int>, int> frow;
+        auto row_of_mask = [&](unsigned mask) -> int {
+            std::map<unsigned, int>::iterator it = vrow.find(mask); if (it != vrow.end()) return it->second;
+            const int id = (int)(P.lanerows.size() / lanes_total); vrow[mask] = id;
+            for (int lane = 0; lane < lanes_total; ++lane) { const int ch = lane / 32, li = lane % 32, h = ch * P.cpc + li; P.lanerows.push_back((li < P.cpc && h < P.NH) ? (uint8_t)extract(cfgbits[h], mask) : 0); }
+            return id;
+        };
+        auto row_of_flags = [&](std::vector<std::pair<int, int> > pairs, int line_leg) -> int {
+            std::sort(pairs.begin(), pairs.end());
+            const std::pair<std::vector<std::pair<int, int> >, int> key(pairs, line_leg);
+            std::map<std::pair<std::vector<std::pair<int, int> >, int>, int>::iterator it = frow.find(key); if (it != frow.end()) return it->second;
+            const int id = (int)(P.lanerows.size() / lanes_total); frow[key] = id;
+            for (int lane = 0; lane < lanes_total; ++lane) {
+                const int ch = lane / 32, li = lane % 32, h = ch * P.cpc + li; uint8_t b = 0;
+                if (li < P.cpc && h < P.NH) {
+                    bool valid = true;
+                    for (size_t q = 0; q < pairs.size(); ++q) if (chi_of_leg(cfgbits[h], pairs[q].first) != chi_of_leg(cfgbits[h], pairs[q].second)) valid = false;
+                    b = (valid ? 1 : 0) | ((line_leg >= 0 && chi_of_leg(cfgbits[h], line_leg) > 0) ? 2 : 0);
+                }
+                P.lanerows.push_back(b);
+            }
+            return id;
+        };
+        // one 16-word record per closing (kind 0-2) or per overflow block of colour updates (kind 3):
+        //  [0] kind | reset S << 2 | updates << 3 | log2 nv of the 4 operands << 8 (3 bits each)   [1] base a | b << 16   [2] base c | d << 16
+        //  [3] variant rows of a, b, c, d (bytes)   [4] flag row | ka << 8 | kb << 16 | kc << 24   [5] coefficient of the amplitude in its group sum
+        //  [6..9] colour updates: J element | coefficient index << 16
+        const int MAXU = 4;
         double fl_b = 0;
+        P.n_entries = 0;
         for (size_t k = 0; k < order.size(); ++k) {
             const int l = order[k]; const Closing& cl = G.closings[l]; const int g = E.group_of[l];
             const bool last = (k + 1 == order.size()) || E.group_of[order[k + 1]] != g;
@@ -295,36 +327,30 @@ struct TabBuilder {
                 else if (cl.piece == 2) { c[1] = cl.c[3]; c[2] = cl.c[1]; c[3] = cl.c[2]; }
             } else if (cl.kind == AK_IOV) { kind = TB_IOV; c[0] = cl.c[1]; c[1] = cl.c[0]; }      // (psi, psibar, gluon)
             else if (cl.kind != AK_VVV) throw std::runtime_error("closing kind without a table form");
-            uint32_t b[4] = {0, 0, 0, 0}, ln[4] = {0, 0, 0, 0}, ks[3] = {0, 0, 0};
-            for (int j = 0; j < 4; ++j) if (c[j] >= 0) { b[j] = (uint32_t)base32[c[j]]; ln[j] = (uint32_t)lognv[c[j]]; }
+            uint32_t b[4] = {0, 0, 0, 0}, ln[4] = {0, 0, 0, 0}, ks[3] = {0, 0, 0}, rows[4] = {0, 0, 0, 0};
+            for (int j = 0; j < 4; ++j) if (c[j] >= 0) { b[j] = (uint32_t)base32[c[j]]; ln[j] = (uint32_t)lognv[c[j]]; rows[j] = (uint32_t)row_of_mask(G.cur[c[j]].varmask); }
             if (kind == TB_VVV) for (int j = 0; j < 3; ++j) { ks[j] = (uint32_t)slot_of(G.cur[c[j]].mask); if (ks[j] > 255) throw std::runtime_error("more than 256 momentum slots"); }
-            uint32_t joff = 0, jcnt = 0;
-            if (last) {
-                joff = (uint32_t)P.jl_index.size(); jcnt = (uint32_t)X[g].size();
-                for (size_t t = 0; t < X[g].size(); ++t) { P.jl_index.push_back((uint16_t)X[g][t].first); P.jl_coef.push_back((uint16_t)coef_of(X[g][t].second)); }
-                fl_b += 4.0 * jcnt;
+            const uint32_t fr = (uint32_t)row_of_flags(cl.pairs, kind == TB_IOV ? G.cur[c[0]].end_leg : -1);
+            const size_t nu = last ? X[g].size() : 0;
+            size_t done = 0;
+            for (int part = 0; part == 0 || done < nu; ++part) {
+                const size_t take = std::min<size_t>(MAXU, nu - done);
+                const bool reset = last && done + take == nu;
+                uint32_t w[16]; memset(w, 0, sizeof w);
+                w[0] = (part == 0 ? (uint32_t)kind : 3u) | ((reset ? 1u : 0u) << 2) | ((uint32_t)take << 3) | (ln[0] << 8) | (ln[1] << 11) | (ln[2] << 14) | (ln[3] << 17);
+                w[1] = b[0] | (b[1] << 16); w[2] = b[2] | (b[3] << 16);
+                w[3] = rows[0] | (rows[1] << 8) | (rows[2] << 16) | (rows[3] << 24);
+                w[4] = fr | (ks[0] << 8) | (ks[1] << 16) | (ks[2] << 24);
+                w[5] = coef_of(E.group_lead[l]);
+                for (size_t t = 0; t < take; ++t) w[6 + t] = (uint32_t)X[g][done + t].first | (coef_of(X[g][done + t].second) << 16);
+                for (int q = 0; q < 16; ++q) P.b_rec.push_back(w[q]);
+                P.n_entries++; done += take; fl_b += 4.0 * take;
             }
-            if (jcnt > 255) throw std::runtime_error("more than 255 colour updates in one group");
-            put4(P.b_entry, b[0] | (b[1] << 16), b[2] | (b[3] << 16),
-                 ln[0] | (ln[1] << 3) | (ln[2] << 6) | (ln[3] << 9) | ((uint32_t)kind << 12) | ((last ? 1u : 0u) << 15) | (ks[0] << 16) | (ks[1] << 24),
-                 ks[2] | (jcnt << 8));
-            put4(P.b_entry, coef_of(E.group_lead[l]), joff, 0, 0);
+            P.n_jl += (int)nu;
             fl_b += FlopTable::of_closing(cl.kind) + 4;
-            int line_leg = -1; if (kind == TB_IOV) line_leg = G.cur[c[0]].end_leg;
-            for (int lane = 0; lane < lanes_total; ++lane) {
-                const int ch = lane / 32, li = lane % 32, h = ch * P.cpc + li;
-                if (li >= P.cpc || h >= P.NH) { P.b_vtab.push_back(0); continue; }
-                const unsigned bits = cfgbits[h];
-                bool valid = true;
-                for (size_t q = 0; q < cl.pairs.size(); ++q) if (chi_of_leg(bits, cl.pairs[q].first) != chi_of_leg(bits, cl.pairs[q].second)) valid = false;
-                uint32_t w = 0;
-                for (int j = 0; j < 4; ++j) if (c[j] >= 0) w |= extract(bits, G.cur[c[j]].varmask) << (5 * j);
-                if (line_leg >= 0 && chi_of_leg(bits, line_leg) > 0) w |= 1u << 20;
-                if (valid) w |= 1u << 21;
-                P.b_vtab.push_back(w);
-            }
         }
-        P.n_jl = (int)P.jl_index.size();
+        if (P.lanerows.size() / lanes_total > 255) throw std::runtime_error("more than 255 lane rows");
+        P.n_rows = (int)(P.lanerows.size() / lanes_total);
         if (P.coef.size() > 65535) throw std::runtime_error("more than 65535 distinct coefficients");
         P.nK = (int)kslot.size();
         P.kmask.assign(P.nK, 0);

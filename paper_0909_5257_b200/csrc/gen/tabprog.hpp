@@ -29,10 +29,9 @@ struct TabProgram {
     std::vector<uint32_t> a_term;       // [n_bterms][32][4] (word 3: index into coef)
     std::vector<uint32_t> a_level;      // [n_levels + 1] bundle ranges
     // phase B (closings, per helicity configuration)
-    std::vector<uint32_t> b_entry;      // [n_closings][8]
-    std::vector<uint32_t> b_vtab;       // [n_closings][nchunks * 32]
-    std::vector<uint16_t> jl_index;     // [n_jl] J element of a group update
-    std::vector<uint16_t> jl_coef;      // [n_jl] index into coef
+    std::vector<uint32_t> b_rec;        // [n_entries][16] closing records (see tab.hpp)
+    std::vector<uint8_t> lanerows;      // [n_rows][nchunks * 32] per-lane bytes: variant of a leg set / validity and chirality flags
+    int n_entries = 0, n_rows = 0;
     std::vector<double> coef;           // pool of the distinct rational coefficients (merged-term weights, group signs, J updates)
     // phase C: colour matrix on the accumulated basis, tiles of 8 rows: cmat[(tile * R + b) * 8 + i] = C[tile*8+i][b] (x2 if b > row, 0 if b < row)
     std::vector<double> cmat;
