@@ -229,7 +229,12 @@ template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, int re
                 ctas = std::min<long>(ctas, 512 / cols);
             }
             const long warps = ctas * w;
-            if (warps > best.warps) { best.epc = epc; best.jm = jm; best.tm_cols = cols; best.tm_wcols = wcols; best.smem = smem; best.warps = warps; }
+            // TMEM bounds the residency but the block scheduler does not know: ask for enough shared memory that no more
+            // CTAs become resident than can allocate their columns (the others would spin inside tcgen05.alloc)
+            size_t ask = smem;
+            if (jm && ctas > 0) ask = std::max<size_t>(smem, (size_t)(228 * 1024) / (ctas + 1) + 1024 - 1024 * 1);
+            if (ask > 227 * 1024) ask = 227 * 1024;
+            if (warps > best.warps) { best.epc = epc; best.jm = jm; best.tm_cols = cols; best.tm_wcols = wcols; best.smem = ask; best.warps = warps; }
         }
     }
     return best;

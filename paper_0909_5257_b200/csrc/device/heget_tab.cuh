@@ -460,25 +460,25 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
         // the closing records stream through a per-warp ring in shared memory, NS - 1 records ahead of their use (cp.async),
         // so the table latency (L2) never shows; operands are fetched one closing ahead of the arithmetic, and the loop is
         // unrolled by two so that the two operand sets alternate without register copies
-        auto issue = [&](int k) {
-            if (lane < ENT / 16) {
+        auto issue2 = [&](int k) {        // records k and k + 1 (k even) in one group
+            if (lane < 2 * (ENT / 16)) {
                 const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + (k & (NS - 1)) * ENT + lane * 16);
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst), "l"(gent + (size_t)k * ENT + lane * 16));
             }
             asm volatile("cp.async.commit_group;\n" ::);
         };
-        auto landed = [&]() { asm volatile("cp.async.wait_group %0;\n" :: "n"(NS - 2)); __syncwarp(); };
+        auto landed = [&]() { asm volatile("cp.async.wait_group 2;\n" ::); __syncwarp(); };
         const int nent = d.n_entries;
-        for (int k = 0; k < NS - 1; ++k) issue(k);           // the table is padded with NS + 2 null records
+        static_assert(HG_TAB_RING == 8, "the prefetch distance below assumes a ring of 8 records");
+        issue2(0); issue2(2); issue2(4);                        // the table is padded with NS + 2 null records
         landed();
         TabOps<T> O0, O1;
         TabCtl<T> C0, C1;
         tab_load_ops<T>(O0, C0, ring, store, evK, myrows);
         for (int k = 0; k < nent; k += 2) {
-            issue(k + NS - 1); landed();
+            issue2(k + 6); landed();                            // records k + 1 and k + 2 are in the ring now
             tab_load_ops<T>(O1, C1, ring + ((k + 1) & (NS - 1)) * ENT, store, evK, myrows);
             tab_finish<T>(O0, C0, ring + (k & (NS - 1)) * ENT, jp, Sr, Si);
-            issue(k + NS); landed();
             tab_load_ops<T>(O0, C0, ring + ((k + 2) & (NS - 1)) * ENT, store, evK, myrows);
             if (k + 1 < nent) tab_finish<T>(O1, C1, ring + ((k + 1) & (NS - 1)) * ENT, jp, Sr, Si);
         }
