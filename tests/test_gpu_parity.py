@@ -76,7 +76,21 @@ def test_rambo_matches_oracle(n_final, sqrt_s, seed):
     # collinear q_i for n = 2): among 2*10^4 events the worst has gamma^2 ~ 10^5, so the bound is on the quantiles.
     assert np.median(d) < 1e-15
     assert np.quantile(d, 0.99) < 1e-13
-    assert d.max() < 1e-9
+    # the tail, event by event: |dp| / sqrt(s) <= 64 eps gamma^2 with the event's own gamma^2 = Q0^2 / M^2, recomputed here from
+    # the oracle's Philox words of the accepted attempt (q0 = -ln(u3 u4), reading A7)
+    eps = 2.0 ** -52
+    tries = tr_o.astype(np.int64)
+    for e in np.nonzero(d > 1e-13)[0]:
+        q = np.zeros((n_final, 4))
+        for i in range(n_final):
+            r = O.philox4x32_10([int(e), 0, int(tries[e] - 1), i], [seed, 0]).astype(np.float64)
+            u = (r + 0.5) / 4294967296.0
+            c, ph, q0 = 2 * u[0] - 1, 2 * math.pi * u[1], -math.log(u[2] * u[3])
+            sn = math.sqrt(1 - c * c)
+            q[i] = [q0, q0 * sn * math.cos(ph), q0 * sn * math.sin(ph), q0 * c]
+        Q = q.sum(axis=0)
+        gamma2 = Q[0] ** 2 / (Q[0] ** 2 - Q[1] ** 2 - Q[2] ** 2 - Q[3] ** 2)
+        assert d[e] <= 64 * eps * gamma2, "event %d: |dp|/sqrt(s) = %.2e, gamma^2 = %.2e" % (e, d[e], gamma2)
     # what holds at any size: momentum conservation, masslessness, beams
     m = mom.cpu().numpy()
     tot = m[2:].sum(axis=0)
@@ -122,12 +136,47 @@ def test_me2_fp32_matches_oracle(events, oracle_process, name, sqrt_s, seed, n):
     mom, mom_h = events(name, sqrt_s, seed, n)
     P = hg.Process(name, sqrt_s, precision="fp32")
     ref = oracle_process(name).me2(mom_h)
-    out = P.eval_me2(mom)
-    assert out.dtype == torch.float32
-    err = rel_err(out.cpu().numpy().astype(np.float64), ref)
-    assert np.all(np.isfinite(err))
-    assert np.median(err) <= TOL32_MEDIAN, "median rel err %.3e" % np.median(err)
-    assert err.max() <= TOL32_MAX, "max rel err %.3e at event %d" % (err.max(), int(err.argmax()))
+    for lanes in sorted({0, 1, P.info.lanes_wide}):          # automatic, one event per thread, wide
+        try:
+            P.set_lanes(lanes)
+        except hg.HegetError as e:
+            assert e.status == hg.EINVAL and lanes == 1 and P.n_ext >= 6
+            continue
+        out = P.eval_me2(mom)
+        assert out.dtype == torch.float32
+        err = rel_err(out.cpu().numpy().astype(np.float64), ref)
+        assert np.all(np.isfinite(err))
+        assert np.median(err) <= TOL32_MEDIAN, "lanes %d: median rel err %.3e" % (lanes, np.median(err))
+        assert err.max() <= TOL32_MAX, "lanes %d: max rel err %.3e at event %d" % (lanes, err.max(), int(err.argmax()))
+
+
+# ---- the table back end: every process, both precisions, J in shared memory and in tensor memory -------------------------------
+TABLE_CASES = CASES + [("u u > u u g g g", 2000.0, 11, 259)]      # NEXT-4: 786 diagrams / 240 colours
+
+
+@pytest.mark.parametrize("jmem", ["smem", "tmem"])
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("name,sqrt_s,seed,n", TABLE_CASES)
+def test_table_kernel_matches_oracle(events, oracle_process, monkeypatch, name, sqrt_s, seed, n, precision, jmem):
+    """heget_set_kernel(TABLE): merged currents, centroid closings, helicity-recycled currents, closings per configuration,
+    J accumulated on the span of the diagrams' colour vectors -- the same |M|^2 as the oracle's plain sum over diagrams."""
+    monkeypatch.setenv("HEGET_TAB_J", jmem)        # read when the handle's launch shape is chosen (first launch)
+    mom, mom_h = events(name, sqrt_s, seed, n)
+    P = hg.Process(name, sqrt_s, precision=precision, kernel="table")
+    assert P.info.kernel == hg.KERNEL_TABLE and P.info.j_in_tmem == (1 if jmem == "tmem" else 0)
+    assert P.info.local_bytes_per_thread == 0
+    ref = oracle_process(name).me2(mom_h)
+    out = P.eval_me2(mom).cpu().numpy().astype(np.float64)
+    err = rel_err(out, ref)
+    if precision == "fp64":
+        assert err.max() <= TOL64, "max rel err %.3e at event %d" % (err.max(), int(err.argmax()))
+    else:
+        assert np.median(err) <= TOL32_MEDIAN and err.max() <= TOL32_MAX, "median %.3e max %.3e" % (np.median(err), err.max())
+    # the two back ends agree with each other far inside the tolerance (same Feynman rules, different organisation of the sum)
+    if P.n_ext <= 6:
+        S = hg.Process(name, sqrt_s, precision=precision, kernel="straight")
+        other = S.eval_me2(mom).cpu().numpy().astype(np.float64)
+        assert rel_err(out, other).max() <= (1e-11 if precision == "fp64" else 2e-4)
 
 
 @pytest.mark.parametrize("name,sqrt_s,seed,n", [c for c in CASES if c[0] in ("u u~ > g g", "g g > g g g")])
@@ -183,7 +232,8 @@ def test_runtime_generated_process(oracle_process, tmp_path, monkeypatch):
 
 
 def test_c1_closed_form(events):
-    """C1 against the textbook result (BASELINE.json configs[0]): me2/S = g^4 [32/27 (t^2+u^2)/(tu) - 8/3 (t^2+u^2)/s^2]."""
+    """C1 against the textbook result (BASELINE.json configs[0]): me2 = 1/2! g^4 [32/27 (t^2+u^2)/(tu) - 8/3 (t^2+u^2)/s^2];
+    the identical-particle factor of the two final gluons is the literal 1/2, not the library's own field."""
     mom, m = events("u u~ > g g", 500.0, 0, 16384)
     P = hg.Process("u u~ > g g", 500.0)
     out = P.eval_me2(mom).cpu().numpy()
@@ -191,7 +241,7 @@ def test_c1_closed_form(events):
     s = 500.0 ** 2
     t = -2 * (m[0, 0] * m[2, 0] - (m[0, 1:] * m[2, 1:]).sum(axis=0))
     u = -2 * (m[0, 0] * m[3, 0] - (m[0, 1:] * m[3, 1:]).sum(axis=0))
-    exact = P.info.sym_factor * g4 * (32.0 / 27.0 * (t * t + u * u) / (t * u) - 8.0 / 3.0 * (t * t + u * u) / s ** 2)
+    exact = 0.5 * g4 * (32.0 / 27.0 * (t * t + u * u) / (t * u) - 8.0 / 3.0 * (t * t + u * u) / s ** 2)
     assert rel_err(out, exact).max() < 1e-11
 
 
@@ -220,24 +270,29 @@ def test_fixed_helicity_mode(events, oracle_process, name, sqrt_s, seed):
     assert rel_err(total, full).max() < 1e-12
 
 
-def test_sampled_helicity_mode(events):
+@pytest.mark.parametrize("kernel", ["straight", "table"])
+def test_sampled_helicity_mode(events, oracle_process, kernel):
     """HEL_SAMPLE (what the paper ran): the value is 2^n_ext times one term of the sum, the draw is
-    reproducible and indexed by the global event, and its mean estimates the helicity sum."""
+    reproducible and indexed by the global event, and its mean estimates the helicity sum.  WHICH configuration event e gets is
+    pinned by the oracle's own Philox4x32-10: counter (e_lo, e_hi, 0xffffffff, 0), key = seed, helicity of leg i = bit
+    (32 - n_ext + i) of the first output word (1 = +1); the value is then 2^n_ext times the oracle's per-helicity colour sum."""
     name, sqrt_s, seed, n = "g g > g g g", 1000.0, 1, 8195
-    mom, _ = events(name, sqrt_s, seed, n)
-    P = hg.Process(name, sqrt_s)
+    mom, mom_h = events(name, sqrt_s, seed, n)
+    P = hg.Process(name, sqrt_s, kernel=kernel)
     a = P.eval_me2(mom, mode=hg.HEL_SAMPLE, seed=11).cpu().numpy()
     b = P.eval_me2(mom, mode=hg.HEL_SAMPLE, seed=11).cpu().numpy()
     assert np.array_equal(a, b)
     c = P.eval_me2(mom[:, :, 100:200].contiguous(), mode=hg.HEL_SAMPLE, seed=11, first_event=100).cpu().numpy()
     assert np.array_equal(c, a[100:200])
-    terms = []
-    for bits in range(32):
+    Po = oracle_process(name)
+    fac = 0.25 / 64.0 / 6.0                      # 1/4 spins, 1/(8*8) colours, 1/3! identical gluons (eqs. 9, 12; PAPER.md:66)
+    for e in list(range(40)) + [4097, 8194]:
+        word = int(O.philox4x32_10([e, 0, 0xffffffff, 0], [11, 0])[0])
+        bits = word >> (32 - 5)
         hel = [1 if (bits >> i) & 1 else -1 for i in range(5)]
-        terms.append(P.eval_me2(mom[:, :, :256].contiguous(), mode=hg.HEL_FIXED, hel=hel).cpu().numpy())
-    terms = np.array(terms) * 32.0
-    for e in range(256):
-        assert np.min(np.abs(terms[:, e] - a[e])) <= 1e-12 * max(a[e], terms[:, e].max())
+        s, _, _ = Po.amplitudes(mom_h[:, :, e].copy(), hel)
+        ref = 32.0 * fac * s
+        assert abs(a[e] - ref) <= 1e-10 * max(ref, 1e-30), "event %d: %g vs %g" % (e, a[e], ref)
     full = P.eval_me2(mom).cpu().numpy()
     ratio = a / full            # E[ratio] = 1 under a uniform helicity draw
     assert abs(ratio.mean() - 1.0) < 5 * ratio.std() / math.sqrt(n)
@@ -284,11 +339,11 @@ def test_no_spill_report_and_launch_counter():
     assert hg.launch_count() == c0 + 2
 
 
-@pytest.mark.parametrize("cfg,precision", [("C2", "fp64"), ("C2", "fp32"), ("C3", "fp64")])
+@pytest.mark.parametrize("cfg,precision", [(c, p) for c in ("C2", "C3", "C4", "C5") for p in ("fp64", "fp32")])
 def test_full_size_bench_configuration(oracle_process, cfg, precision):
-    """BASELINE.json's full size in the launch configuration bench.py times (automatic lanes): sampled events against the
-    oracle one by one, plus what holds at any size -- every |M|^2 positive and finite, and Bose symmetry: exchanging the momenta
-    of two identical final-state gluons leaves |M|^2 unchanged (SURVEY.md 8(c) 'permutation symmetry')."""
+    """BASELINE.json's full size in the launch configuration bench.py times (automatic back end and lanes): sampled events
+    against the oracle one by one, plus what holds at any size -- every |M|^2 positive and finite, and Bose symmetry: exchanging
+    the momenta of two identical final-state gluons leaves |M|^2 unchanged (SURVEY.md 8(c) 'permutation symmetry')."""
     from bench import CONFIGS
     name, sqrt_s, E, seed = CONFIGS[cfg]
     P = hg.Process(name, sqrt_s, precision=precision)
@@ -307,8 +362,12 @@ def test_full_size_bench_configuration(oracle_process, cfg, precision):
     swapped = mom.clone()
     swapped[a], swapped[b] = mom[b], mom[a]
     out2 = P.eval_me2(swapped)
-    sym = ((out2 - out).abs() / out).max().item()
-    assert sym <= (1e-11 if precision == "fp64" else 1e-3)
+    sym = ((out2 - out).abs() / out)
+    # a symmetry bound, not the accuracy tolerance: the two evaluations differ only in the order of the same FP operations
+    if precision == "fp64":
+        assert sym.max().item() <= 1e-11
+    else:
+        assert sym.median().item() <= 1e-6 and sym.max().item() <= 1e-4
 
 
 @pytest.mark.parametrize("name,sqrt_s,seed", [("g g > g g g g", 1500.0, 3), ("u u~ > g g g g", 1500.0, 9)])

@@ -50,6 +50,41 @@ def test_two_to_two_closed_forms(oracle_process, name):
         assert abs(me[e] / P.sym_factor / ref - 1.0) < 1e-12
 
 
+# identical-particle factors 1/prod k! as BASELINE.json's config strings print them: "1/2!" (C1 by the closed form
+# below), "1/3!", "1/2! 1/2!", "1/4!", "1/5!"; plus two processes that tell "u and u~ counted together" and "initial legs
+# counted" apart.  Mutations this fails: counting u and u~ as identical (u u~ > u u~ would give 1/2), including the initial
+# legs (g g > g g g would give 1/5!), forgetting the factor (1).
+SYM_LITERALS = {
+    "u u~ > g g": 1.0 / 2.0, "g g > g g g": 1.0 / 6.0, "u u > u u g g": 1.0 / 4.0, "g g > g g g g": 1.0 / 24.0,
+    "u u~ > g g g g g": 1.0 / 120.0, "u u~ > u u~": 1.0, "u u > u u": 1.0 / 2.0, "u g > u g g": 1.0 / 2.0, "u u~ > d d~": 1.0,
+}
+
+
+@pytest.mark.parametrize("name", sorted(SYM_LITERALS))
+def test_identical_particle_factor_literals(oracle_process, name):
+    assert oracle_process(name).sym_factor == SYM_LITERALS[name]
+
+
+def test_c1_absolute_value(oracle_process):
+    """The oracle's me2 for BASELINE.json configs[0] itself -- factor included, nothing divided out:
+    me2 = (1/2) g^4 [32/27 (t^2+u^2)/(tu) - 8/3 (t^2+u^2)/s^2] with g^2 = 4 pi 0.118 (the literal 1/2 is the 1/2! of P:66)."""
+    P = oracle_process("u u~ > g g")
+    mom, _, _ = O.sample_momenta(2, 500.0, 0, 256)
+    me = P.me2(mom)
+    g4 = (4.0 * np.pi * 0.118) ** 2
+    for e in range(256):
+        s, t, u = mandelstam(mom, e)
+        ref = 0.5 * g4 * (32 / 27 * (t * t + u * u) / (t * u) - 8 / 3 * (t * t + u * u) / s ** 2)
+        assert abs(me[e] / ref - 1.0) < 1e-12
+    # and for identical quarks: 1/2! times the textbook u u -> u u result
+    Q = oracle_process("u u > u u")
+    mq = Q.me2(mom)
+    for e in range(64):
+        s, t, u = mandelstam(mom, e)
+        ref = 0.5 * g4 * (4 / 9 * ((s * s + u * u) / t ** 2 + (s * s + t * t) / u ** 2) - 8 / 27 * s * s / (t * u))
+        assert abs(mq[e] / ref - 1.0) < 1e-12
+
+
 def all_outgoing(p):
     k = p.copy()
     k[:2] *= -1.0

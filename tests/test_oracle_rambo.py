@@ -73,6 +73,28 @@ def test_rambo_isotropy_without_cuts():
     assert abs(mom[2:, 0].mean() - 1000.0 / 3.0) < 1e-9
 
 
+def test_rambo_energy_law_three_body():
+    """Flat massless 3-body phase space: x_i = 2 E_i / sqrt(s) has the marginal density 2x on [0, 1] (the Dalitz triangle
+    x_1 + x_2 + x_3 = 2 is uniformly populated), so <E^2> = s/8 and, with sum E = sqrt(s), <E_i E_j> = 5 s / 48 for i != j.
+    <E> = sqrt(s)/3 holds by symmetry for ANY q0 law, so it pins nothing; these second moments do: drawing q0 = -ln(u3)
+    instead of -ln(u3 u4) (reading A7) gives <E^2> = 0.1313 s (and P(x < 1/2) = 0.277) -- about 39 sigma away at this sample size."""
+    n = 200000
+    s = 1000.0 ** 2
+    mom, w, tries = O.sample_momenta(3, 1000.0, 12, n, pt_min=0.0, eta_max=0.0, dr_min=0.0)
+    E = mom[2:, 0]                                  # [3, n]
+    x = 2.0 * E / 1000.0
+    # var(x^2) under density 2x: <x^4> - <x^2>^2 = 1/3 - 1/4 = 1/12
+    for i in range(3):
+        assert abs((E[i] ** 2).mean() - s / 8.0) < 5.0 * (s / 4.0) * math.sqrt(1.0 / 12.0 / n)
+    for i in range(3):
+        for j in range(i + 1, 3):
+            prod = x[i] * x[j]
+            assert abs(prod.mean() - 5.0 / 12.0) < 5.0 * prod.std() / math.sqrt(n)
+    # the whole marginal, not only its moments: P(x < 1/2) = 1/4, P(x < 0.9) = 0.81
+    for q, pr in [(0.5, 0.25), (0.9, 0.81)]:
+        assert abs((x[0] < q).mean() - pr) < 5.0 * math.sqrt(pr * (1 - pr) / n)
+
+
 def test_event_index_is_global_counter():
     # reading A17/A18: event e of a batch starting at first_event equals event first_event+e of a batch from 0
     a, wa, ta = O.sample_momenta(3, 1000.0, 1, 64, first_event=0)
