@@ -2,9 +2,12 @@
 
     python oracle/build.py
 
-Compiles oracle/oracle_api.cpp with g++ (-O2, OpenMP, IEEE arithmetic: no -ffast-math) into
-oracle/liboracle.so.  Called by __graft_entry__.build() and, lazily, by oracle/oracle.py.
+Compiles oracle/oracle_api.cpp with g++ (-O3 -march=native as BASELINE.md section 3 states for the timed CPU baseline, OpenMP,
+IEEE arithmetic: no -ffast-math) into oracle/liboracle.so.  Called by __graft_entry__.build() and, lazily, by oracle/oracle.py.
+The library is specific to the CPU it was built on: a stamp (flags of this CPU + the command line) sits beside it, and a
+library carried over from another machine (the GPU box receives this tree) is rebuilt there.
 """
+import hashlib
 import os
 import subprocess
 import sys
@@ -15,8 +18,28 @@ HDR = ["su3.hpp", "kin.hpp", "rambo.hpp", "diagrams.hpp", "colour.hpp", "eval.hp
 LIB = os.path.join(HERE, "liboracle.so")
 
 
+STAMP = os.path.join(HERE, "liboracle.stamp")
+CMD = ["g++", "-std=c++17", "-O3", "-march=native", "-fopenmp", "-fPIC", "-shared", "-Wall"]
+
+
+def _stamp():
+    flags = ""
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("flags") or line.startswith("model name"):
+                    flags += line
+                    if line.startswith("flags"):
+                        break
+    except OSError:
+        pass
+    return hashlib.sha256((flags + " ".join(CMD)).encode()).hexdigest()
+
+
 def needs_build():
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
+        return True
+    if open(STAMP).read().strip() != _stamp():
         return True
     t = os.path.getmtime(LIB)
     return any(os.path.getmtime(os.path.join(HERE, f)) > t for f in SRC + HDR)
@@ -25,9 +48,11 @@ def needs_build():
 def build(force=False):
     if not force and not needs_build():
         return LIB
-    cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall",
-           "-o", LIB] + [os.path.join(HERE, s) for s in SRC]
-    subprocess.check_call(cmd, cwd=HERE)
+    tmp = LIB + ".%d.tmp" % os.getpid()
+    subprocess.check_call(CMD + ["-o", tmp] + [os.path.join(HERE, s) for s in SRC], cwd=HERE)
+    os.replace(tmp, LIB)
+    with open(STAMP, "w") as f:
+        f.write(_stamp() + "\n")
     return LIB
 
 

@@ -83,7 +83,7 @@ double orc_me2(void* h, const double* mom, uint64_t n_events, int tier, int n_th
     const int n = M->D.proc.n_ext();
     if (n_threads > 0) omp_set_num_threads(n_threads);
     auto t0 = std::chrono::steady_clock::now();
-    #pragma omp parallel for schedule(dynamic, 1)
+    #pragma omp parallel for schedule(static)
     for (int64_t e = 0; e < (int64_t)n_events; ++e) {
         double p[16][4]; gather(mom, n_events, (uint64_t)e, n, p);
         out[e] = me2_event(*M, p, tier);
