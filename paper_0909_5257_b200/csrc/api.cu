@@ -414,7 +414,7 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
     if (effective_kernel(p) == HEGET_KERNEL_TABLE) {
         const heget::TabProgram& t = *p->tab;
         o->kernel = HEGET_KERNEL_TABLE;
-        o->n_ext = t.n_ext; o->n_hel = t.n_hel; o->n_hel_eval = t.NH; o->n_diagrams = t.n_diagrams; o->n_topologies = t.n_topologies;
+        o->n_ext = t.n_ext; o->n_hel = t.n_hel; o->n_hel_eval = t.n_hel_nonzero; o->n_hel_computed = t.NH; o->n_diagrams = t.n_diagrams; o->n_topologies = t.n_topologies;
         o->n_color = t.n_color; o->n_color_eval = t.n_color_eval; o->n_color_reduced = t.NJ; o->n_color_accum = t.R; o->color_rank = t.color_rank;
         o->avg_spin = t.avg_spin; o->avg_color = t.avg_color; o->sym_factor = t.sym_factor;
         o->flops_per_event = t.flops_per_event; o->flops_per_helicity = t.flops_per_hel;
@@ -434,7 +434,7 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
     }
     const hg::ProcDesc* d = p->d;
     o->kernel = HEGET_KERNEL_STRAIGHT;
-    o->n_ext = d->n_ext; o->n_hel = d->n_hel; o->n_hel_eval = d->n_hel_eval; o->n_diagrams = d->n_diagrams; o->n_topologies = d->n_topologies;
+    o->n_ext = d->n_ext; o->n_hel = d->n_hel; o->n_hel_eval = d->n_hel_eval; o->n_hel_computed = d->n_hel_eval; o->n_diagrams = d->n_diagrams; o->n_topologies = d->n_topologies;
     o->n_color = d->n_color; o->n_color_eval = d->n_color_eval; o->n_color_reduced = d->n_color_reduced; o->n_color_accum = d->n_color_reduced;
     if (p->tab) o->color_rank = p->tab->color_rank;
     o->avg_spin = d->avg_spin; o->avg_color = d->avg_color; o->sym_factor = d->sym_factor;
@@ -506,10 +506,11 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
     int hel_fixed = -1;
     if (mode == HEGET_HEL_FIXED) {
         for (int i = 0; i < n_ext; ++i) if (hel[i] != 1 && hel[i] != -1) return fail(HEGET_EINVAL, "heget_eval_me2: hel[%d] = %d is not +-1", i, (int)hel[i]);
+        const bool folded = table && p->tab->hel_weight == 2;
         for (int h = 0; h < n_eval && hel_fixed < 0; ++h) {
-            bool same = true;
-            for (int i = 0; i < n_ext; ++i) if (htab[h * n_ext + i] != hel[i]) { same = false; break; }
-            if (same) hel_fixed = h;
+            bool same = true, mirror = folded;
+            for (int i = 0; i < n_ext; ++i) { if (htab[h * n_ext + i] != hel[i]) same = false; if (htab[h * n_ext + i] != -hel[i]) mirror = false; }
+            if (same || mirror) hel_fixed = h;
         }
     }
     if (table) {
@@ -522,7 +523,9 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         cudaStream_t s = (cudaStream_t)cuda_stream;
         const TabShape& sh = p->tab_shape;
         const double iss = 1.0 / p->sqrt_s;
-#define HG_TAB_LAUNCH(TT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)blocks, threads, sh.smem, s>>>(p->tdev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, iss, p->out_scale, (TT*)d_me2, (int)mode, hel_fixed, seed, first_event)
+        // parity-folded helicity sum: every evaluated configuration stands for itself and its mirror image
+        const double oscale = p->out_scale * (mode == HEGET_HEL_SUM ? (double)p->tab->hel_weight : 1.0);
+#define HG_TAB_LAUNCH(TT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)blocks, threads, sh.smem, s>>>(p->tdev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, iss, oscale, (TT*)d_me2, (int)mode, hel_fixed, seed, first_event)
         if (p->prec == HEGET_FP64) { if (sh.jm) HG_TAB_LAUNCH(double, 1); else HG_TAB_LAUNCH(double, 0); }
         else { if (sh.jm) HG_TAB_LAUNCH(float, 1); else HG_TAB_LAUNCH(float, 0); }
 #undef HG_TAB_LAUNCH

@@ -1,6 +1,7 @@
 // In-process entry to the process generator (step a0), used by
 // heget_process_create when no pre-built plug-in exists for a process.  Same work as the hegetgen command line.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <fstream>
 #include "emit.hpp"
@@ -80,6 +81,7 @@ heget::TabProgram* heget_build_table(const char* tag, const char* process, int* 
         } catch (std::exception& e) { snprintf(msg, msglen, "%s", e.what()); *rc = 2; return 0; }
         if (G.closings.empty()) { snprintf(msg, msglen, "process has no tree-level QCD diagram"); *rc = 2; return 0; }
         TabBuilder B(G, tag);
+        { const char* f = getenv("HEGET_TAB_FOLD"); if (f && f[0] == '0') B.fold_parity = false; }      // HEGET_TAB_FOLD=0: evaluate both members of every parity pair
         B.build(paper);
         const Graph& GC = paper ? *paper : G;
         B.P.color_rank = rank_mod_p(GC.C, (int)GC.basis.size());

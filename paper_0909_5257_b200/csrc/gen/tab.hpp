@@ -115,6 +115,7 @@ struct TabBuilder {
         const uint32_t id = (uint32_t)P.coef.size(); P.coef.push_back(f.value()); coef_index[key] = id; return id;
     }
 
+    bool fold_parity = true;
     void build(const Graph* paper, bool allow_rank_reduction = true) {
         const int n = G.P.n;
         P.name = G.P.name; P.tag = E.tag; P.n_ext = n; P.n_hel = 1 << n;
@@ -122,7 +123,15 @@ struct TabBuilder {
         chisign.assign(n, 0);
         for (int i = 0; i < n; ++i) if (G.P.legs[i].type != LEG_G) chisign[i] = G.P.legs[i].anti ? +1 : -1;      // Emitter::chi_of: chi = -h (anti: +h)
         E.analyse_helicities(); E.reduce_colour(); E.build_groups();
-        P.n_gluons = E.ng; P.n_quark_legs = E.nq; P.NH = E.NH; P.NJ = E.NJ;
+        P.n_gluons = E.ng; P.n_quark_legs = E.nq; P.NJ = E.NJ;
+        // Parity folding of the helicity sum (eq. 12): QCD conserves parity, so |M|^2 of a configuration equals that of the
+        // configuration with every helicity flipped (the oracle pins this per configuration, tests/test_oracle_amplitudes.py).
+        // The non-vanishing configurations come in such pairs; one of each pair (leg 0 at helicity -1) is evaluated and counted
+        // twice.  HEL_FIXED / HEL_SAMPLE map a requested configuration onto its evaluated partner.
+        std::vector<int> kept;
+        for (int h = 0; h < E.NH; ++h) if (!fold_parity || E.hel_of(h)[0] < 0) kept.push_back(h);
+        if (fold_parity && 2 * (int)kept.size() != E.NH) throw std::runtime_error("helicity configurations are not closed under parity");
+        P.NH = (int)kept.size(); P.n_hel_nonzero = E.NH; P.hel_weight = fold_parity ? 2 : 1;
         P.nchunks = (P.NH + 31) / 32; P.cpc = (P.NH + P.nchunks - 1) / P.nchunks;
         P.n_diagrams = (int)std::lround(G.n_diagrams_paper); P.n_topologies = (int)std::lround(G.n_topologies);
         const Graph& GP = paper ? *paper : G;
@@ -283,7 +292,12 @@ struct TabBuilder {
         const int lanes_total = P.nchunks * 32;
         std::vector<unsigned> cfgbits(P.NH, 0);
         P.hel_table.assign((size_t)P.NH * n, 0); P.evalidx.assign((size_t)1 << n, -1);
-        for (int h = 0; h < P.NH; ++h) { std::vector<int> hv = E.hel_of(h); for (int i = 0; i < n; ++i) { P.hel_table[(size_t)h * n + i] = (int8_t)hv[i]; if (hv[i] > 0) cfgbits[h] |= 1u << i; } P.evalidx[cfgbits[h]] = (int16_t)h; }
+        for (int h = 0; h < P.NH; ++h) {
+            std::vector<int> hv = E.hel_of(kept[h]);
+            for (int i = 0; i < n; ++i) { P.hel_table[(size_t)h * n + i] = (int8_t)hv[i]; if (hv[i] > 0) cfgbits[h] |= 1u << i; }
+            P.evalidx[cfgbits[h]] = (int16_t)h;
+            if (fold_parity) P.evalidx[~cfgbits[h] & ((1u << n) - 1u)] = (int16_t)h;
+        }
         // per-lane byte rows (one byte per helicity configuration of every warp): row of a leg set = the variant index the
         // configuration selects in a current over those legs; row of (quark-line pairing, line) = bit 0: the configuration
         // conserves chirality along the closing's quark lines, bit 1: chirality of the closing's own line

@@ -13,6 +13,7 @@ enum TabKindB { TB_VVV = 0, TB_GGGG = 1, TB_IOV = 2 };
 struct TabProgram {
     std::string name, tag;
     int n_ext = 0, n_gluons = 0, n_quark_legs = 0;
+    int n_hel_nonzero = 0, hel_weight = 1;             // configurations that do not vanish identically; 2 if the sum is parity-folded
     int NH = 0, n_hel = 0, nchunks = 0, cpc = 0;       // evaluated configurations, 2^n, warps per event, configurations per warp
     int NJ = 0, R = 0, Rpad = 0;                       // merged colour basis, rank actually accumulated, padded to tiles of 8
     int nK = 0, store32 = 0;                           // momentum slots, store size in 16-byte chunks of the FP32 layout
