@@ -273,7 +273,7 @@ static heget_status_t table_to_device(heget_process* p) {
         const size_t npad = (size_t)t.n_entries + HG_TAB_RING + 2;
         std::vector<unsigned char> ent(npad * ENT, 0);
         for (size_t k = 0; k < npad; ++k) {
-            uint32_t w[28]; memset(w, 0, sizeof w);
+            uint32_t w[32]; memset(w, 0, sizeof w);
             if (k >= (size_t)t.n_entries) { w[0] = 3u; memcpy(&ent[k * ENT], w, ENT); continue; }      // null record: no amplitude, no update
             const uint32_t* e = &t.b_rec[k * 16];
             const unsigned kind = e[0] & 3u, reset = (e[0] >> 2) & 1u, nu = (e[0] >> 3) & 7u;
@@ -330,6 +330,9 @@ extern "C" {
 
 const char* heget_last_error(void) { return g_err; }
 uint64_t heget_launch_count(void) { return g_launches.load(); }
+#ifdef HG_TAB_TIMING
+void heget_debug_timing(unsigned long long* out, int reset) { cudaDeviceSynchronize(); cudaMemcpyFromSymbol(out, hg::g_tab_timing, 64); if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(hg::g_tab_timing, z, 64); } }
+#endif
 
 heget_status_t heget_fma_probe(heget_precision_t prec, uint64_t iters, void* d_out, uint64_t n_threads, double* flops, void* cuda_stream) {
     if (!d_out || !flops || n_threads == 0 || n_threads % 256) return fail(HEGET_EINVAL, "heget_fma_probe: d_out/flops NULL or n_threads not a multiple of 256");

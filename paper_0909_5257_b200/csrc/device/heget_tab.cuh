@@ -46,8 +46,9 @@ template <typename T> __host__ __device__ inline size_t tab_event_bytes(int nK, 
     return (size_t)nK * 4 * sizeof(T) + (((size_t)nK * sizeof(T) + 15) / 16) * 16 + (size_t)store32 * 16 * (sizeof(T) / 4);
 }
 template <typename T> __host__ __device__ inline size_t tab_warp_bytes(int R) { return (size_t)2 * R * 32 * sizeof(T); }
-// a closing record is 64 bytes in FP32 (16 words) and 112 bytes in FP64; every warp keeps TAB_RING of them in flight
-template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { return sizeof(T) == 4 ? 64 : 112; }
+// a closing record is 64 bytes in FP32 (16 words) and 128 bytes in FP64 (112 used); every warp keeps TAB_RING of them in flight.
+// After phase B the ring double-buffers the blocks of the colour matrix (64 coefficients = 256 / 512 bytes each).
+template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { return sizeof(T) == 4 ? 64 : 128; }
 #define HG_TAB_RING 8
 template <typename T> __host__ __device__ inline size_t tab_rows_bytes(int n_rows, int nchunks) { return (((size_t)n_rows * nchunks * 32) + 15) / 16 * 16; }
 template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, bool j_in_tmem = false) {
@@ -56,6 +57,9 @@ template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, boo
 }
 
 #if defined(__CUDACC__)
+#ifdef HG_TAB_TIMING
+__device__ unsigned long long g_tab_timing[8];
+#endif
 template <typename T> struct tabio;
 template <> struct tabio<float> {
     static __device__ __forceinline__ vec4<float> ldv(const unsigned char* st, unsigned addr, unsigned lnv) {
@@ -350,6 +354,9 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     const bool live = e < n_events;
     if (!live) e = n_events - 1;
 
+#ifdef HG_TAB_TIMING
+    long long tt0 = clock64(), tt1, tt2, tt3 = 0, tt4;
+#endif
     const T* cf = reinterpret_cast<const T*>(d.coef);
     // ---- prologue ------------------------------------------------------------------------------------------------------
     for (int c = tid; c < 4 * n * epc; c += blockDim.x) {
@@ -392,6 +399,9 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     }
     __syncthreads();
 
+#ifdef HG_TAB_TIMING
+    tt1 = clock64();
+#endif
     // ---- phase A: off-shell currents, once per helicity variant ----------------------------------------------------------
     for (int lev = 0; lev < d.n_levels; ++lev) {
         const int b1 = (int)__ldg(d.a_level + lev + 1);
@@ -437,6 +447,9 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
         __syncthreads();
     }
 
+#ifdef HG_TAB_TIMING
+    tt2 = clock64();
+#endif
     // ---- phase B: closings, one helicity configuration per lane -------------------------------------------------------------
     const int h = wie * d.cpc + lane;
     const bool hvalid = lane < d.cpc && h < d.NH;
@@ -486,43 +499,70 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
             }
         }
         asm volatile("cp.async.wait_all;\n" ::);
+#ifdef HG_TAB_TIMING
+        tt3 = clock64();
+#endif
         // ---- phase C: colour form on the accumulated basis ----------------------------------------------------------------
+        // t_a = C_aa J_a + sum_{b > a} 2 C_ab J_b for a tile of 8 rows stays in registers while J streams through (from shared
+        // memory or TMEM) in blocks of 8 columns.  The 8 x 8 coefficient block of each step comes through the warp's ring
+        // (free after phase B) by cp.async, one block ahead, so the latency of the matrix (L2) is hidden.
         const T* cm = reinterpret_cast<const T*>(d.cmat);
-        for (int t = 0; t < d.Rpad / 8; ++t) {
+        const int ntile = d.Rpad / 8;
+        constexpr int CB = 64 * sizeof(T);                    // bytes of one coefficient block
+        __syncwarp();
+        auto fetch = [&](int t, int bb, int buf) {
+            if (lane < CB / 16 && t < ntile) {
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + buf * CB + lane * 16);
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(cm + ((size_t)t * d.Rpad + (size_t)8 * bb) * 8) + lane * 16;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst), "l"(src));
+            }
+            asm volatile("cp.async.commit_group;\n" ::);
+        };
+        int buf = 0;
+        fetch(0, 0, 0);
+        for (int t = 0; t < ntile; ++t) {
             T tr[8], ti[8], dr[8], di[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) { tr[i] = T(0); ti[i] = T(0); }
-            const T* row = cm + (size_t)t * R * 8;
-            for (int bb = t; bb < d.Rpad / 8; ++bb) {
+            for (int bb = t; bb < ntile; ++bb) {
+                // next block: (t, bb + 1), or the first block of the next tile (nothing after the last one: an empty group)
+                const bool last_bb = bb + 1 == ntile;
+                fetch(last_bb ? t + 1 : t, last_bb ? t + 1 : bb + 1, buf ^ 1);
                 T xr[8], xi[8];
                 jp.block8(8 * bb, R, xr, xi);
                 if (bb == t) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i) { dr[i] = xr[i]; di[i] = xi[i]; }
                 }
+                asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp();
+                const T* cblk = reinterpret_cast<const T*>(ring + buf * CB);
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
-                    const int b = 8 * bb + q;
-                    if (b < R) {
-                        T c8[8];
-                        if constexpr (sizeof(T) == 4) {
-                            const float4 c0 = __ldg(reinterpret_cast<const float4*>(row + (size_t)b * 8)), c1 = __ldg(reinterpret_cast<const float4*>(row + (size_t)b * 8) + 1);
-                            c8[0] = c0.x; c8[1] = c0.y; c8[2] = c0.z; c8[3] = c0.w; c8[4] = c1.x; c8[5] = c1.y; c8[6] = c1.z; c8[7] = c1.w;
-                        } else {
-                            const double2* rp = reinterpret_cast<const double2*>(row + (size_t)b * 8);
-                            const double2 c0 = __ldg(rp), c1 = __ldg(rp + 1), c2 = __ldg(rp + 2), c3 = __ldg(rp + 3);
-                            c8[0] = c0.x; c8[1] = c0.y; c8[2] = c1.x; c8[3] = c1.y; c8[4] = c2.x; c8[5] = c2.y; c8[6] = c3.x; c8[7] = c3.y;
-                        }
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) { tr[i] += c8[i] * xr[q]; ti[i] += c8[i] * xi[q]; }
+                    T c8[8];
+                    if constexpr (sizeof(T) == 4) {
+                        const float4 c0 = *reinterpret_cast<const float4*>(cblk + q * 8), c1 = *reinterpret_cast<const float4*>(cblk + q * 8 + 4);
+                        c8[0] = c0.x; c8[1] = c0.y; c8[2] = c0.z; c8[3] = c0.w; c8[4] = c1.x; c8[5] = c1.y; c8[6] = c1.z; c8[7] = c1.w;
+                    } else {
+                        const double2* rp = reinterpret_cast<const double2*>(cblk + q * 8);
+                        const double2 c0 = rp[0], c1 = rp[1], c2 = rp[2], c3 = rp[3];
+                        c8[0] = c0.x; c8[1] = c0.y; c8[2] = c1.x; c8[3] = c1.y; c8[4] = c2.x; c8[5] = c2.y; c8[6] = c3.x; c8[7] = c3.y;
                     }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) { tr[i] += c8[i] * xr[q]; ti[i] += c8[i] * xi[q]; }
                 }
+                __syncwarp();
+                buf ^= 1;
             }
 #pragma unroll
             for (int i = 0; i < 8; ++i) form += dr[i] * tr[i] + di[i] * ti[i];
         }
+        asm volatile("cp.async.wait_all;\n" ::);
     }
     // ---- helicity sum (eq. 12) and averaging factors -------------------------------------------------------------
+#ifdef HG_TAB_TIMING      // debug build only: cycles per phase, summed over warps
+    tt4 = clock64();
+    if (lane == 0 && chunk_on) { atomicAdd(&g_tab_timing[0], (unsigned long long)(tt1 - tt0)); atomicAdd(&g_tab_timing[1], (unsigned long long)(tt2 - tt1)); atomicAdd(&g_tab_timing[2], (unsigned long long)(tt3 - tt2)); atomicAdd(&g_tab_timing[3], (unsigned long long)(tt4 - tt3)); atomicAdd(&g_tab_timing[4], 1ull); }
+#endif
     T acc = wgt * form;          // the helicity sum stays in the kernel's own precision (reading A21)
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (lane == 0) red[el * wpe + wie] = (double)acc;

@@ -185,10 +185,11 @@ struct TabBuilder {
         }
         P.Rpad = (P.R + 7) / 8 * 8;
         for (size_t a = 0; a < cacc.size(); ++a) P.colour_acc.push_back(cacc[a].value());
-        P.cmat.assign((size_t)(P.Rpad / 8) * P.R * 8, 0.0);
+        // tiles of 8 rows, Rpad columns each (columns beyond R are zero), one more tile of zeros at the end (the kernel prefetches one block ahead)
+        P.cmat.assign((size_t)(P.Rpad / 8 + 1) * P.Rpad * 8, 0.0);
         for (int t = 0; t < P.Rpad / 8; ++t) for (int b = 0; b < P.R; ++b) for (int i = 0; i < 8; ++i) {
             const int a = t * 8 + i; if (a >= P.R || b < a) continue;
-            P.cmat[((size_t)t * P.R + b) * 8 + i] = cacc[(size_t)a * P.R + b].value() * (b > a ? 2.0 : 1.0);
+            P.cmat[((size_t)t * P.Rpad + b) * 8 + i] = cacc[(size_t)a * P.R + b].value() * (b > a ? 2.0 : 1.0);
         }
 
         // ---- store layout: every current holds 2^|varmask| variants of 4 (gluon) or 2 (Weyl spinor) complex components ----

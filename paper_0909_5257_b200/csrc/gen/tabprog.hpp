@@ -34,7 +34,7 @@ struct TabProgram {
     std::vector<uint8_t> lanerows;      // [n_rows][nchunks * 32] per-lane bytes: variant of a leg set / validity and chirality flags
     int n_entries = 0, n_rows = 0;
     std::vector<double> coef;           // pool of the distinct rational coefficients (merged-term weights, group signs, J updates)
-    // phase C: colour matrix on the accumulated basis, tiles of 8 rows: cmat[(tile * R + b) * 8 + i] = C[tile*8+i][b] (x2 if b > row, 0 if b < row)
+    // phase C: colour matrix on the accumulated basis, tiles of 8 rows: cmat[(tile * Rpad + b) * 8 + i] = C[tile*8+i][b] (x2 if b > row, 0 if b < row or b >= R), plus one tile of zeros
     std::vector<double> cmat;
     // host-side info
     std::vector<int8_t> hel_table;      // [NH][n]
