@@ -86,6 +86,7 @@ typedef struct {
     int kernel;                /* back end the next heget_eval_me2 takes: HEGET_KERNEL_STRAIGHT or HEGET_KERNEL_TABLE */
     int events_per_block;
     int n_hel_computed;        /* configurations the kernel actually evaluates: n_hel_eval, or half of it when the TABLE back end folds the sum by parity (|M|^2 is invariant under flipping every helicity; each evaluated configuration counts twice) */
+    int packed_pairs;          /* TABLE back end, FP32: 1 if two events share a warp on packed f32x2 instructions (FFMA2) */
     int j_in_tmem;             /* TABLE back end: 1 if the warps keep their J in tensor memory (TMEM), 0 = shared memory */
     double flops_per_event_tensor; /* flops of the colour stage executed on the tensor pipe (0: vector pipes)        */
 } heget_info_t;

@@ -140,6 +140,7 @@ __global__ void __launch_bounds__(256) k_fma_probe(T* out, unsigned long long it
 }  // namespace
 
 struct TabShape { int epc, jm, tm_cols, tm_wcols; size_t smem; long warps; };
+enum TabElem { TE_F64 = 0, TE_F32 = 1, TE_F32X2 = 2 };      // element type of the table kernels: double, float, packed pair of floats (two events)
 struct heget_process;
 static int effective_lanes(const heget_process* p);
 
@@ -149,7 +150,7 @@ static int effective_lanes(const heget_process* p);
 struct heget_process {
     const hg::ProcDesc* d;
     heget::TabProgram* tab;
-    hg::TabDev tdev; bool tab_on_device; std::vector<void*> tab_allocs; int tab_epc; TabShape tab_shape;
+    hg::TabDev tdev; bool tab_on_device; std::vector<void*> tab_allocs; int tab_epc; TabShape tab_shape; int tab_elem;
     std::string name, tag;
     int n_legs, kernel_req;        // requested back end: HEGET_KERNEL_AUTO / STRAIGHT / TABLE
     bool auto_table;               // what AUTO means for this process
@@ -247,13 +248,21 @@ template <typename T, int JM> static int tab_kernel_regs() {
     if (cudaFuncGetAttributes(&fa, hg::k_tab<T, JM>) != cudaSuccess) { cudaGetLastError(); return 0; }
     return fa.numRegs;
 }
-static TabShape tab_shape_of(const hg::TabDev& d, int prec) {
-    return prec == HEGET_FP64 ? tab_pick_shape<double>(d, tab_kernel_regs<double, 0>(), tab_kernel_regs<double, 1>())
-                              : tab_pick_shape<float>(d, tab_kernel_regs<float, 0>(), tab_kernel_regs<float, 1>());
+// FP32 handles run the table program on packed f32x2 arithmetic, two events per warp (HEGET_TAB_PACK=0: scalar, one event per warp)
+static int tab_elem_of(int prec) {
+    if (prec == HEGET_FP64) return TE_F64;
+    const char* e = getenv("HEGET_TAB_PACK");
+    return (e && e[0] == '0') ? TE_F32 : TE_F32X2;
+}
+static TabShape tab_shape_of(const hg::TabDev& d, int elem) {
+    if (elem == TE_F64) return tab_pick_shape<double>(d, tab_kernel_regs<double, 0>(), tab_kernel_regs<double, 1>());
+    if (elem == TE_F32) return tab_pick_shape<float>(d, tab_kernel_regs<float, 0>(), tab_kernel_regs<float, 1>());
+    return tab_pick_shape<hg::f2>(d, tab_kernel_regs<hg::f2, 0>(), tab_kernel_regs<hg::f2, 1>());
 }
 
 static heget_status_t table_to_device(heget_process* p) {
     if (p->tab_on_device) return HEGET_OK;
+    p->tab_elem = tab_elem_of(p->prec);
     const heget::TabProgram& t = *p->tab;
     hg::TabDev& d = p->tdev;
     memset(&d, 0, sizeof d);
@@ -267,7 +276,9 @@ static heget_status_t table_to_device(heget_process* p) {
     if ((st = upload(p, t.a_term, &d.a_term)) != HEGET_OK) return st;
     if ((st = upload(p, t.a_level, &d.a_level)) != HEGET_OK) return st;
     {   // closing records in the byte layout of this precision (heget_tab.cuh, tab_load_ops / tab_finish)
-        const bool f64 = p->prec == HEGET_FP64;
+        const bool f64 = p->tab_elem != TE_F32;       // 8-byte elements: double, or a pair of floats
+        const bool pairf = p->tab_elem == TE_F32X2;
+        auto enc8 = [&](double c, void* dst) { if (pairf) { const float f[2] = {(float)c, (float)c}; memcpy(dst, f, 8); } else memcpy(dst, &c, 8); };
         const unsigned scale = f64 ? 2u : 1u, esz = f64 ? 8u : 4u;
         const size_t ENT = f64 ? hg::tab_entry_bytes<double>() : hg::tab_entry_bytes<float>(), LT = (size_t)t.nchunks * 32;
         const size_t npad = (size_t)t.n_entries + HG_TAB_RING + 2;
@@ -289,8 +300,8 @@ static heget_status_t table_to_device(heget_process* p) {
             w[6] = ka | (kb << 16);
             const double sgn = t.coef[e[5]];
             if (f64) {
-                memcpy(&w[8], &sgn, 8);
-                for (unsigned j = 0; j < nu; ++j) { const double c = t.coef[e[6 + j] >> 16]; w[12 + 4 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 8u; memcpy(&w[14 + 4 * j], &c, 8); }
+                enc8(sgn, &w[8]);
+                for (unsigned j = 0; j < nu; ++j) { const double c = t.coef[e[6 + j] >> 16]; w[12 + 4 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 8u; enc8(c, &w[14 + 4 * j]); }
             } else {
                 const float sf = (float)sgn; memcpy(&w[7], &sf, 4);
                 for (unsigned j = 0; j < nu; ++j) { const float c = (float)t.coef[e[6 + j] >> 16]; w[8 + 2 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 4u; memcpy(&w[9 + 2 * j], &c, 4); }
@@ -303,20 +314,29 @@ static heget_status_t table_to_device(heget_process* p) {
         d.n_entries = t.n_entries; d.n_rows = t.n_rows;
     }
     if ((st = upload(p, t.evalidx, &d.evalidx)) != HEGET_OK) return st;
-    if (p->prec == HEGET_FP64) {
+    if (p->tab_elem == TE_F64) {
         const double* c = 0; if ((st = upload(p, t.cmat, &c)) != HEGET_OK) return st; d.cmat = c;
         if ((st = upload(p, t.coef, &c)) != HEGET_OK) return st; d.coef = c;
-    } else {
+    } else if (p->tab_elem == TE_F32) {
         std::vector<float> cm(t.cmat.begin(), t.cmat.end()), cf(t.coef.begin(), t.coef.end()); const float* c = 0;
         if ((st = upload(p, cm, &c)) != HEGET_OK) return st; d.cmat = c;
         if ((st = upload(p, cf, &c)) != HEGET_OK) return st; d.coef = c;
+    } else {      // both halves of a packed value hold the same coefficient
+        std::vector<float> cm(2 * t.cmat.size()), cf(2 * t.coef.size()); const float* c = 0;
+        for (size_t i = 0; i < t.cmat.size(); ++i) cm[2 * i] = cm[2 * i + 1] = (float)t.cmat[i];
+        for (size_t i = 0; i < t.coef.size(); ++i) cf[2 * i] = cf[2 * i + 1] = (float)t.coef[i];
+        if ((st = upload(p, cm, &c)) != HEGET_OK) return st; d.cmat = c;
+        if ((st = upload(p, cf, &c)) != HEGET_OK) return st; d.coef = c;
     }
-    p->tab_shape = tab_shape_of(d, p->prec);
+    p->tab_shape = tab_shape_of(d, p->tab_elem);
     if (p->tab_shape.epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
     p->tab_epc = p->tab_shape.epc;
     const int smem = (int)p->tab_shape.smem;
-    if (p->prec == HEGET_FP64) { if (p->tab_shape.jm) CU(cudaFuncSetAttribute(hg::k_tab<double, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); else CU(cudaFuncSetAttribute(hg::k_tab<double, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); }
-    else { if (p->tab_shape.jm) CU(cudaFuncSetAttribute(hg::k_tab<float, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); else CU(cudaFuncSetAttribute(hg::k_tab<float, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); }
+#define HG_TAB_ATTR(TT, JMV) CU(cudaFuncSetAttribute(hg::k_tab<TT, JMV>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem))
+    if (p->tab_elem == TE_F64) { if (p->tab_shape.jm) HG_TAB_ATTR(double, 1); else HG_TAB_ATTR(double, 0); }
+    else if (p->tab_elem == TE_F32) { if (p->tab_shape.jm) HG_TAB_ATTR(float, 1); else HG_TAB_ATTR(float, 0); }
+    else { if (p->tab_shape.jm) HG_TAB_ATTR(hg::f2, 1); else HG_TAB_ATTR(hg::f2, 0); }
+#undef HG_TAB_ATTR
     p->tab_on_device = true;
     return HEGET_OK;
 }
@@ -424,13 +444,15 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
         o->lanes_wide = 32; o->lanes = 32;
         hg::TabDev d; memset(&d, 0, sizeof d); d.n_ext = t.n_ext; d.nchunks = t.nchunks; d.R = t.R; d.nK = t.nK; d.store32 = t.store32; d.n_rows = t.n_rows;
         d.Rpad = t.Rpad;
-        const TabShape sh = tab_shape_of(d, p->prec);
-        o->events_per_block = sh.epc; o->threads_per_block = sh.epc * t.nchunks * 32; o->j_in_tmem = sh.jm;
+        const int elem = tab_elem_of(p->prec);
+        const TabShape sh = tab_shape_of(d, elem);
+        o->events_per_block = sh.epc * (elem == TE_F32X2 ? 2 : 1); o->threads_per_block = sh.epc * t.nchunks * 32; o->j_in_tmem = sh.jm; o->packed_pairs = elem == TE_F32X2;
         if (have_dev) {
             cudaFuncAttributes fa;
             cudaError_t e;
-            if (p->prec == HEGET_FP64) e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<double, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<double, 0>);
-            else e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<float, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<float, 0>);
+            if (elem == TE_F64) e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<double, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<double, 0>);
+            else if (elem == TE_F32) e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<float, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<float, 0>);
+            else e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<hg::f2, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<hg::f2, 0>);
             if (e == cudaSuccess) { o->regs_per_thread = fa.numRegs; o->local_bytes_per_thread = (int)fa.localSizeBytes; } else cudaGetLastError();
         }
         return HEGET_OK;
@@ -520,7 +542,8 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         const heget_status_t st = table_to_device(p);
         if (st != HEGET_OK) return st;
         const int epc = p->tab_epc;
-        const unsigned long long blocks = (n_events + epc - 1) / epc;
+        const int evpc = epc * (p->tab_elem == TE_F32X2 ? 2 : 1);       // events per CTA
+        const unsigned long long blocks = (n_events + evpc - 1) / evpc;
         if (blocks > 0x7fffffffull) return fail(HEGET_EINVAL, "heget_eval_me2: n_events too large for one launch");
         const int threads = epc * p->tdev.nchunks * 32;
         cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -528,9 +551,10 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         const double iss = 1.0 / p->sqrt_s;
         // parity-folded helicity sum: every evaluated configuration stands for itself and its mirror image
         const double oscale = p->out_scale * (mode == HEGET_HEL_SUM ? (double)p->tab->hel_weight : 1.0);
-#define HG_TAB_LAUNCH(TT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)blocks, threads, sh.smem, s>>>(p->tdev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, iss, oscale, (TT*)d_me2, (int)mode, hel_fixed, seed, first_event)
-        if (p->prec == HEGET_FP64) { if (sh.jm) HG_TAB_LAUNCH(double, 1); else HG_TAB_LAUNCH(double, 0); }
-        else { if (sh.jm) HG_TAB_LAUNCH(float, 1); else HG_TAB_LAUNCH(float, 0); }
+#define HG_TAB_LAUNCH(TT, OT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)blocks, threads, sh.smem, s>>>(p->tdev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, iss, oscale, (OT*)d_me2, (int)mode, hel_fixed, seed, first_event)
+        if (p->tab_elem == TE_F64) { if (sh.jm) HG_TAB_LAUNCH(double, double, 1); else HG_TAB_LAUNCH(double, double, 0); }
+        else if (p->tab_elem == TE_F32) { if (sh.jm) HG_TAB_LAUNCH(float, float, 1); else HG_TAB_LAUNCH(float, float, 0); }
+        else { if (sh.jm) HG_TAB_LAUNCH(hg::f2, float, 1); else HG_TAB_LAUNCH(hg::f2, float, 0); }
 #undef HG_TAB_LAUNCH
         CU(cudaGetLastError());
         g_launches++;

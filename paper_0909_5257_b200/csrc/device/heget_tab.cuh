@@ -52,7 +52,8 @@ template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { retu
 #define HG_TAB_RING 8
 template <typename T> __host__ __device__ inline size_t tab_rows_bytes(int n_rows, int nchunks) { return (((size_t)n_rows * nchunks * 32) + 15) / 16 * 16; }
 template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, bool j_in_tmem = false) {
-    return (size_t)epc * (sizeof(double) * 4 * d.n_ext + tab_event_bytes<T>(d.nK, d.store32) + (size_t)d.nchunks * ((j_in_tmem ? 0 : tab_warp_bytes<T>(d.R)) + HG_TAB_RING * tab_entry_bytes<T>()) + sizeof(double) * d.nchunks)
+    const int ev = sizeof(T) == 8 && !std::is_same<T, double>::value ? 2 : 1;      // events per slot
+    return (size_t)epc * (sizeof(double) * 4 * d.n_ext * ev + tab_event_bytes<T>(d.nK, d.store32) + (size_t)d.nchunks * ((j_in_tmem ? 0 : tab_warp_bytes<T>(d.R)) + HG_TAB_RING * tab_entry_bytes<T>()) + sizeof(double) * d.nchunks * ev)
            + tab_rows_bytes<T>(d.n_rows, d.nchunks);
 }
 
@@ -60,7 +61,62 @@ template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, boo
 #ifdef HG_TAB_TIMING
 __device__ unsigned long long g_tab_timing[8];
 #endif
-template <typename T> struct tabio;
+// ---- element traits ------------------------------------------------------------------------------------------------------------
+// T = double: FP64.  T = float: FP32, one event per warp.  T = f2 (heget_dev.cuh): FP32 on packed f32x2 instructions (FFMA2 / FMUL2 /
+// FADD2), the two halves being TWO EVENTS that walk the table together: every arithmetic instruction, every table word, every address
+// computation serves both, which halves the issue slots per event of a kernel that is issue-bound in FP32.
+template <typename T> struct el;
+template <> struct el<float> {
+    static constexpr int EV = 1; typedef float out_t;
+    static __device__ __forceinline__ float pack(double a, double) { return (float)a; }
+    static __device__ __forceinline__ float half(float v, int) { return v; }
+};
+template <> struct el<double> {
+    static constexpr int EV = 1; typedef double out_t;
+    static __device__ __forceinline__ double pack(double a, double) { return a; }
+    static __device__ __forceinline__ double half(double v, int) { return v; }
+    static __device__ __forceinline__ double from_bits(unsigned lo, unsigned hi) { return __hiloint2double((int)hi, (int)lo); }
+    static __device__ __forceinline__ unsigned lo(double v) { return (unsigned)__double2loint(v); }
+    static __device__ __forceinline__ unsigned hi(double v) { return (unsigned)__double2hiint(v); }
+};
+template <> struct el<f2> {
+    static constexpr int EV = 2; typedef float out_t;
+    static __device__ __forceinline__ f2 pack(double a, double b) { return f2((float)a, (float)b); }
+    static __device__ __forceinline__ float half(f2 v, int j) { return j ? v.hi() : v.lo(); }
+    static __device__ __forceinline__ f2 from_bits(unsigned lo, unsigned hi) { f2 r; r.v = ((unsigned long long)hi << 32) | lo; return r; }
+    static __device__ __forceinline__ unsigned lo(f2 v) { return (unsigned)v.v; }
+    static __device__ __forceinline__ unsigned hi(f2 v) { return (unsigned)(v.v >> 32); }
+};
+template <typename T> __device__ __forceinline__ cx<T> cx_bits(const uint4 u) { return mk<T>(el<T>::from_bits(u.x, u.y), el<T>::from_bits(u.z, u.w)); }
+template <typename T> __device__ __forceinline__ uint4 bits_cx(const cx<T>& c) { return make_uint4(el<T>::lo(c.re), el<T>::hi(c.re), el<T>::lo(c.im), el<T>::hi(c.im)); }
+
+template <typename T> struct tabio {       // 8-byte elements (double, f2): one complex per 16-byte chunk
+    // chunk of (current base32 b, variant v): 2 b + q nv + v; addr = b + v with b a multiple of nv
+    static __device__ __forceinline__ unsigned a64(unsigned addr, unsigned lnv) { const unsigned m = (1u << lnv) - 1u; return 2u * (addr & ~m) + (addr & m); }
+    static __device__ __forceinline__ vec4<T> ldv(const unsigned char* st, unsigned addr, unsigned lnv) {
+        const uint4* s = reinterpret_cast<const uint4*>(st) + a64(addr, lnv);
+        const unsigned nv = 1u << lnv;
+        vec4<T> w; w.v[0] = cx_bits<T>(s[0]); w.v[1] = cx_bits<T>(s[nv]); w.v[2] = cx_bits<T>(s[2 * nv]); w.v[3] = cx_bits<T>(s[3 * nv]); return w;
+    }
+    static __device__ __forceinline__ void stv(unsigned char* st, unsigned addr, unsigned lnv, const vec4<T>& w) {
+        uint4* s = reinterpret_cast<uint4*>(st) + a64(addr, lnv);
+        const unsigned nv = 1u << lnv;
+        s[0] = bits_cx<T>(w.v[0]); s[nv] = bits_cx<T>(w.v[1]); s[2 * nv] = bits_cx<T>(w.v[2]); s[3 * nv] = bits_cx<T>(w.v[3]);
+    }
+    static __device__ __forceinline__ sp2<T> lds(const unsigned char* st, unsigned addr, unsigned lnv) {
+        const uint4* s = reinterpret_cast<const uint4*>(st) + a64(addr, lnv);
+        sp2<T> f; f.s[0] = cx_bits<T>(s[0]); f.s[1] = cx_bits<T>(s[1u << lnv]); return f;
+    }
+    static __device__ __forceinline__ void sts(unsigned char* st, unsigned addr, unsigned lnv, const sp2<T>& f) {
+        uint4* s = reinterpret_cast<uint4*>(st) + a64(addr, lnv);
+        s[0] = bits_cx<T>(f.s[0]); s[1u << lnv] = bits_cx<T>(f.s[1]);
+    }
+    static __device__ __forceinline__ mom4<T> ldk(const T* evk, unsigned slot) {
+        const uint4* s = reinterpret_cast<const uint4*>(evk) + 2 * slot;
+        const uint4 c0 = s[0], c1 = s[1];
+        mom4<T> k; k.p[0] = el<T>::from_bits(c0.x, c0.y); k.p[1] = el<T>::from_bits(c0.z, c0.w); k.p[2] = el<T>::from_bits(c1.x, c1.y); k.p[3] = el<T>::from_bits(c1.z, c1.w); return k;
+    }
+};
 template <> struct tabio<float> {
     static __device__ __forceinline__ vec4<float> ldv(const unsigned char* st, unsigned addr, unsigned lnv) {
         const float4* s = reinterpret_cast<const float4*>(st);
@@ -83,35 +139,6 @@ template <> struct tabio<float> {
         mom4<float> k; k.p[0] = c.x; k.p[1] = c.y; k.p[2] = c.z; k.p[3] = c.w; return k;
     }
 };
-template <> struct tabio<double> {
-    // FP64 chunk of (current base32 b, variant v): 2 b + q nv + v; addr = b + v with b a multiple of nv
-    static __device__ __forceinline__ unsigned a64(unsigned addr, unsigned lnv) { const unsigned m = (1u << lnv) - 1u; return 2u * (addr & ~m) + (addr & m); }
-    static __device__ __forceinline__ vec4<double> ldv(const unsigned char* st, unsigned addr, unsigned lnv) {
-        const double2* s = reinterpret_cast<const double2*>(st) + a64(addr, lnv);
-        const unsigned nv = 1u << lnv;
-        const double2 c0 = s[0], c1 = s[nv], c2 = s[2 * nv], c3 = s[3 * nv];
-        vec4<double> w; w.v[0] = mk<double>(c0.x, c0.y); w.v[1] = mk<double>(c1.x, c1.y); w.v[2] = mk<double>(c2.x, c2.y); w.v[3] = mk<double>(c3.x, c3.y); return w;
-    }
-    static __device__ __forceinline__ void stv(unsigned char* st, unsigned addr, unsigned lnv, const vec4<double>& w) {
-        double2* s = reinterpret_cast<double2*>(st) + a64(addr, lnv);
-        const unsigned nv = 1u << lnv;
-        s[0] = make_double2(w.v[0].re, w.v[0].im); s[nv] = make_double2(w.v[1].re, w.v[1].im); s[2 * nv] = make_double2(w.v[2].re, w.v[2].im); s[3 * nv] = make_double2(w.v[3].re, w.v[3].im);
-    }
-    static __device__ __forceinline__ sp2<double> lds(const unsigned char* st, unsigned addr, unsigned lnv) {
-        const double2* s = reinterpret_cast<const double2*>(st) + a64(addr, lnv);
-        const double2 c0 = s[0], c1 = s[1u << lnv];
-        sp2<double> f; f.s[0] = mk<double>(c0.x, c0.y); f.s[1] = mk<double>(c1.x, c1.y); return f;
-    }
-    static __device__ __forceinline__ void sts(unsigned char* st, unsigned addr, unsigned lnv, const sp2<double>& f) {
-        double2* s = reinterpret_cast<double2*>(st) + a64(addr, lnv);
-        s[0] = make_double2(f.s[0].re, f.s[0].im); s[1u << lnv] = make_double2(f.s[1].re, f.s[1].im);
-    }
-    static __device__ __forceinline__ mom4<double> ldk(const double* evk, unsigned slot) {
-        const double2* s = reinterpret_cast<const double2*>(evk) + 2 * slot;
-        const double2 c0 = s[0], c1 = s[1];
-        mom4<double> k; k.p[0] = c0.x; k.p[1] = c0.y; k.p[2] = c1.x; k.p[3] = c1.y; return k;
-    }
-};
 
 template <typename T> __device__ __forceinline__ void vacc(vec4<T>& a, const vec4<T>& b) {
 #pragma unroll
@@ -127,20 +154,21 @@ template <typename T> __device__ __forceinline__ void sacc(sp2<T>& a, const sp2<
 // IOV w[0..1] = psi, w[2..3] = psibar, w[4..7] = gluon
 template <typename T> struct TabOps { cx<T> w[16]; T k[12]; };
 
-template <typename T> __device__ __forceinline__ void tab_ld(cx<T>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp);
+template <typename T> __device__ __forceinline__ void tab_ld(cx<T>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp) {      // 8-byte elements
+    const uint4* s = reinterpret_cast<const uint4*>(store) + addr;
+    w[0] = cx_bits<T>(s[0]); w[1] = cx_bits<T>(s[stride]);
+    if (ncomp == 4) { w[2] = cx_bits<T>(s[2 * stride]); w[3] = cx_bits<T>(s[3 * stride]); }
+}
 template <> __device__ __forceinline__ void tab_ld<float>(cx<float>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp) {
     const float4* s = reinterpret_cast<const float4*>(store) + addr;
     const float4 c0 = s[0]; w[0] = mk<float>(c0.x, c0.y); w[1] = mk<float>(c0.z, c0.w);
     if (ncomp == 4) { const float4 c1 = s[stride]; w[2] = mk<float>(c1.x, c1.y); w[3] = mk<float>(c1.z, c1.w); }
 }
-template <> __device__ __forceinline__ void tab_ld<double>(cx<double>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp) {
-    const double2* s = reinterpret_cast<const double2*>(store) + addr;
-    const double2 c0 = s[0], c1 = s[stride]; w[0] = mk<double>(c0.x, c0.y); w[1] = mk<double>(c1.x, c1.y);
-    if (ncomp == 4) { const double2 c2 = s[2 * stride], c3 = s[3 * stride]; w[2] = mk<double>(c2.x, c2.y); w[3] = mk<double>(c3.x, c3.y); }
+template <typename T> __device__ __forceinline__ void tab_ldk4(T* k, const T* p) {      // 8-byte elements
+    const uint4 c0 = reinterpret_cast<const uint4*>(p)[0], c1 = reinterpret_cast<const uint4*>(p)[1];
+    k[0] = el<T>::from_bits(c0.x, c0.y); k[1] = el<T>::from_bits(c0.z, c0.w); k[2] = el<T>::from_bits(c1.x, c1.y); k[3] = el<T>::from_bits(c1.z, c1.w);
 }
-template <typename T> __device__ __forceinline__ void tab_ldk4(T* k, const T* p);
 template <> __device__ __forceinline__ void tab_ldk4<float>(float* k, const float* p) { const float4 c = *reinterpret_cast<const float4*>(p); k[0] = c.x; k[1] = c.y; k[2] = c.z; k[3] = c.w; }
-template <> __device__ __forceinline__ void tab_ldk4<double>(double* k, const double* p) { const double2 c0 = reinterpret_cast<const double2*>(p)[0], c1 = reinterpret_cast<const double2*>(p)[1]; k[0] = c0.x; k[1] = c0.y; k[2] = c1.x; k[3] = c1.y; }
 // closing record (uniform, in the warp's ring).  Word 0: kind (0 vvv, 1 gggg, 2 iov, 3 updates only) | reset S << 2 | updates << 3 |
 // byte offset of the flag row << 16; words 1-2: chunk bases of the operands a | b << 16, c | d << 16; words 3-4: byte offsets of their
 // variant rows; word 5: strides (chunks between the 16-byte pieces of one variant) a | b << 8 | c << 16 | d << 24; word 6: byte offsets
@@ -153,7 +181,7 @@ template <typename T> __device__ __forceinline__ void tab_load_ops(TabOps<T>& O,
     const unsigned kind = q0.x & 3u;
     C.ctl = q0.x;
     T sgc;
-    if constexpr (sizeof(T) == 4) sgc = __uint_as_float(q1.w); else sgc = *reinterpret_cast<const double*>(ent + 32);
+    if constexpr (sizeof(T) == 4) sgc = __uint_as_float(q1.w); else { const uint2 sb = *reinterpret_cast<const uint2*>(ent + 32); sgc = el<T>::from_bits(sb.x, sb.y); }
     const unsigned fb = myrows[q0.x >> 16];
     C.sg = (fb & 1u) ? sgc : T(0); C.chi = (fb & 2u) != 0u;
     if (kind == 3u) return;
@@ -237,9 +265,33 @@ template <typename T> struct JSmem {
         for (int i = 0; i < 8; ++i) { const bool in = k0 + i < R; xr[i] = in ? J[(2 * (k0 + i)) * 32] : T(0); xi[i] = in ? J[(2 * (k0 + i) + 1) * 32] : T(0); }
     }
 };
-template <typename T> struct JTmem;
-template <> struct JTmem<float> {
+template <typename T> struct JTmem {       // 8-byte elements: 4 columns per complex number
     unsigned ta;      // TMEM address of column 0 of this warp's block (lane field = first lane of the warp's quadrant)
+    __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st4(ta + 4 * k, 0u, 0u, 0u, 0u); tm_wait_st(); }
+    __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
+        unsigned r[4][4];
+        tm_wait_st();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (j < nu) tm_ld4(ta + (off[j] >> 7), r[j][0], r[j][1], r[j][2], r[j][3]);
+        tm_wait_ld();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (j < nu) {
+            const T re = el<T>::from_bits(r[j][0], r[j][1]) + c[j] * Sr, im = el<T>::from_bits(r[j][2], r[j][3]) + c[j] * Si;
+            tm_st4(ta + (off[j] >> 7), el<T>::lo(re), el<T>::hi(re), el<T>::lo(im), el<T>::hi(im));
+        }
+    }
+    __device__ __forceinline__ void block8(int k0, int, T* xr, T* xi) {
+        unsigned r[8][4];
+        tm_wait_st();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) tm_ld4(ta + 4 * (k0 + i), r[i][0], r[i][1], r[i][2], r[i][3]);
+        tm_wait_ld();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { xr[i] = el<T>::from_bits(r[i][0], r[i][1]); xi[i] = el<T>::from_bits(r[i][2], r[i][3]); }
+    }
+};
+template <> struct JTmem<float> {
+    unsigned ta;
     __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st2(ta + 2 * k, 0u, 0u); tm_wait_st(); }
     __device__ __forceinline__ void update(int nu, const unsigned* off, const float* c, float Sr, float Si) {
         unsigned r[4][2];
@@ -258,31 +310,6 @@ template <> struct JTmem<float> {
         tm_wait_ld();
 #pragma unroll
         for (int i = 0; i < 8; ++i) { xr[i] = __uint_as_float(r[i][0]); xi[i] = __uint_as_float(r[i][1]); }
-    }
-};
-template <> struct JTmem<double> {
-    unsigned ta;
-    __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st4(ta + 4 * k, 0u, 0u, 0u, 0u); tm_wait_st(); }
-    __device__ __forceinline__ void update(int nu, const unsigned* off, const double* c, double Sr, double Si) {
-        unsigned r[4][4];
-        tm_wait_st();
-#pragma unroll
-        for (int j = 0; j < 4; ++j) if (j < nu) tm_ld4(ta + (off[j] >> 7), r[j][0], r[j][1], r[j][2], r[j][3]);
-        tm_wait_ld();
-#pragma unroll
-        for (int j = 0; j < 4; ++j) if (j < nu) {
-            const double re = __hiloint2double((int)r[j][1], (int)r[j][0]) + c[j] * Sr, im = __hiloint2double((int)r[j][3], (int)r[j][2]) + c[j] * Si;
-            tm_st4(ta + (off[j] >> 7), (unsigned)__double2loint(re), (unsigned)__double2hiint(re), (unsigned)__double2loint(im), (unsigned)__double2hiint(im));
-        }
-    }
-    __device__ __forceinline__ void block8(int k0, int, double* xr, double* xi) {
-        unsigned r[8][4];
-        tm_wait_st();
-#pragma unroll
-        for (int i = 0; i < 8; ++i) tm_ld4(ta + 4 * (k0 + i), r[i][0], r[i][1], r[i][2], r[i][3]);
-        tm_wait_ld();
-#pragma unroll
-        for (int i = 0; i < 8; ++i) { xr[i] = __hiloint2double((int)r[i][1], (int)r[i][0]); xi[i] = __hiloint2double((int)r[i][3], (int)r[i][2]); }
     }
 };
 
@@ -305,7 +332,7 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_finish(co
             off[2] = u1.x; c[2] = __uint_as_float(u1.y); off[3] = u1.z; c[3] = __uint_as_float(u1.w);
         } else {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) { const uint4 uu = *reinterpret_cast<const uint4*>(ent + 48 + 16 * j); off[j] = uu.x; c[j] = __hiloint2double((int)uu.w, (int)uu.z); }
+            for (int j = 0; j < 4; ++j) { const uint4 uu = *reinterpret_cast<const uint4*>(ent + 48 + 16 * j); off[j] = uu.x; c[j] = el<T>::from_bits(uu.z, uu.w); }
         }
         jp.update(nu, off, c, Sr, Si);
     }
@@ -315,7 +342,7 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_finish(co
 // JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp)
 template <typename T, int JM>
 __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long n_events,
-        const double inv_sqrt_s, const double out_scale, T* __restrict__ me2, const int hel_mode, const int hel_fixed,
+        const double inv_sqrt_s, const double out_scale, typename el<T>::out_t* __restrict__ me2, const int hel_mode, const int hel_fixed,
         const unsigned long long seed, const unsigned long long first_event) {
     typedef tabio<T> IO;
     extern __shared__ __align__(16) unsigned char hg_tab_smem[];
@@ -323,9 +350,9 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     const int tid = threadIdx.x, el = tid / tpe, te = tid % tpe, wie = te >> 5, lane = tid & 31;
     // carve: [pm: double 4n x epc][red: double epc x wpe][per event: evK | evI | store][per warp: J]
     double* pm = reinterpret_cast<double*>(hg_tab_smem);
-    double* red = pm + (size_t)4 * n * epc;
+    double* red = pm + (size_t)4 * n * epc * hg::el<T>::EV;
     const size_t evb = tab_event_bytes<T>(d.nK, d.store32);
-    unsigned char* evbase = reinterpret_cast<unsigned char*>(red + (size_t)epc * wpe);
+    unsigned char* evbase = reinterpret_cast<unsigned char*>(red + (size_t)epc * wpe * hg::el<T>::EV);
     evbase += (16 - ((size_t)(evbase - hg_tab_smem) & 15)) & 15;
     unsigned char* myev = evbase + (size_t)el * evb;
     T* evK = reinterpret_cast<T*>(myev);
@@ -349,19 +376,20 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     }
     for (int c = tid; c < (d.n_rows * wpe * 32 + 3) / 4; c += blockDim.x) reinterpret_cast<unsigned int*>(rows)[c] = __ldg(reinterpret_cast<const unsigned int*>(d.lanerows) + c);
 
-    const unsigned long long e0 = (unsigned long long)blockIdx.x * epc;
-    unsigned long long e = e0 + el;
-    const bool live = e < n_events;
-    if (!live) e = n_events - 1;
+    // a slot of the CTA holds EV events (2 for the packed type: they travel in the two halves of every value)
+    constexpr int EV = hg::el<T>::EV;
+    const unsigned long long e0 = (unsigned long long)blockIdx.x * epc * EV;
+    const unsigned long long e = e0 + (unsigned long long)el * EV;
 
 #ifdef HG_TAB_TIMING
     long long tt0 = clock64(), tt1, tt2, tt3 = 0, tt4;
 #endif
     const T* cf = reinterpret_cast<const T*>(d.coef);
     // ---- prologue ------------------------------------------------------------------------------------------------------
-    for (int c = tid; c < 4 * n * epc; c += blockDim.x) {
-        unsigned long long ee = e0 + (unsigned long long)(c % epc); if (ee >= n_events) ee = n_events - 1;
-        pm[c] = mom[(size_t)(c / epc) * n_events + ee] * inv_sqrt_s;
+    const int epe = epc * EV;
+    for (int c = tid; c < 4 * n * epe; c += blockDim.x) {
+        unsigned long long ee = e0 + (unsigned long long)(c % epe); if (ee >= n_events) ee = n_events - 1;
+        pm[c] = mom[(size_t)(c / epe) * n_events + ee] * inv_sqrt_s;
     }
     __syncthreads();
     if constexpr (JM == 1) {
@@ -370,30 +398,63 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
         jp.ta = tm_base + ((unsigned)((wic & 3) * 32) << 16) + (unsigned)((wic >> 2) * tm_wcols);
     }
     {
-        const double* pe = pm + el;
+        typedef hg::el<T> EL;
+        const double* pe = pm + el * EV;             // component c of the slot's event j: pe[c * epe + j]
         for (int s = te; s < d.nK; s += tpe) {       // momentum of a leg subset, all momenta flowing INTO the diagram, and 1/q^2
             const unsigned mask = __ldg(d.kmask + s);
-            double k0 = 0, k1 = 0, k2 = 0, k3 = 0;
-            for (int i = 0; i < n; ++i) if ((mask >> i) & 1u) {
-                const double sg = i < 2 ? 1.0 : -1.0;
-                k0 += sg * pe[(4 * i) * epc]; k1 += sg * pe[(4 * i + 1) * epc]; k2 += sg * pe[(4 * i + 2) * epc]; k3 += sg * pe[(4 * i + 3) * epc];
+            double k[2][4], iq[2];
+#pragma unroll
+            for (int j = 0; j < EV; ++j) {
+                double k0 = 0, k1 = 0, k2 = 0, k3 = 0;
+                for (int i = 0; i < n; ++i) if ((mask >> i) & 1u) {
+                    const double sg = i < 2 ? 1.0 : -1.0;
+                    k0 += sg * pe[(4 * i) * epe + j]; k1 += sg * pe[(4 * i + 1) * epe + j]; k2 += sg * pe[(4 * i + 2) * epe + j]; k3 += sg * pe[(4 * i + 3) * epe + j];
+                }
+                k[j][0] = k0; k[j][1] = k1; k[j][2] = k2; k[j][3] = k3;
+                iq[j] = (mask & (mask - 1u)) ? 1.0 / (k0 * k0 - k1 * k1 - k2 * k2 - k3 * k3) : 0.0;
             }
-            evK[4 * s] = (T)k0; evK[4 * s + 1] = (T)k1; evK[4 * s + 2] = (T)k2; evK[4 * s + 3] = (T)k3;
-            evI[s] = (mask & (mask - 1u)) ? (T)(1.0 / (k0 * k0 - k1 * k1 - k2 * k2 - k3 * k3)) : T(0);
+            constexpr int J1 = EV - 1;
+#pragma unroll
+            for (int m = 0; m < 4; ++m) evK[4 * s + m] = EL::pack(k[0][m], k[J1][m]);
+            evI[s] = EL::pack(iq[0], iq[J1]);
         }
         for (int i = te; i < n; i += tpe) {           // external wavefunctions, both helicities (variant 0: h = -1, variant 1: h = +1)
             const unsigned info = __ldg(d.leginfo + i), ty = info & 0xffu, base = info >> 16;
-            const double p[4] = {pe[(4 * i) * epc], pe[(4 * i + 1) * epc], pe[(4 * i + 2) * epc], pe[(4 * i + 3) * epc]};
+            constexpr int J1 = EV - 1;
+            double b[2][6];
+#pragma unroll
+            for (int j = 0; j < EV; ++j) {
+                const double p[4] = {pe[(4 * i) * epe + j], pe[(4 * i + 1) * epe + j], pe[(4 * i + 2) * epe + j], pe[(4 * i + 3) * epe + j]};
+                if (ty < 2u) vxxxxx_basis<double>(p, ty == 1u, b[j], b[j] + 3); else ixxxxx_basis<double>(p, b[j]);
+            }
             if (ty < 2u) {
-                double r[3], q[3]; vxxxxx_basis<double>(p, ty == 1u, r, q);
-                const T rt[3] = {(T)r[0], (T)r[1], (T)r[2]}, qt[3] = {(T)q[0], (T)q[1], (T)q[2]};
+                const T rt[3] = {EL::pack(b[0][0], b[J1][0]), EL::pack(b[0][1], b[J1][1]), EL::pack(b[0][2], b[J1][2])};
+                const T qt[3] = {EL::pack(b[0][3], b[J1][3]), EL::pack(b[0][4], b[J1][4]), EL::pack(b[0][5], b[J1][5])};
                 IO::stv(store, base, 1, vxxxxx<T>(rt, qt, T(-1))); IO::stv(store, base + 1, 1, vxxxxx<T>(rt, qt, T(1)));
             } else {
-                double s3[3]; ixxxxx_basis<double>(p, s3);
-                const T st3[3] = {(T)s3[0], (T)s3[1], (T)s3[2]};
                 const T cs = ((info >> 8) & 1u) ? T(1) : T(-1);      // chirality = cs * helicity
-                if (ty == 2u) { IO::sts(store, base, 1, ixxxxx<T>(st3, -cs)); IO::sts(store, base + 1, 1, ixxxxx<T>(st3, cs)); }
-                else          { IO::sts(store, base, 1, oxxxxx<T>(st3, -cs)); IO::sts(store, base + 1, 1, oxxxxx<T>(st3, cs)); }
+                if constexpr (EV == 1) {
+                    const T st3[3] = {EL::pack(b[0][0], 0.0), EL::pack(b[0][1], 0.0), EL::pack(b[0][2], 0.0)};
+                    if (ty == 2u) { IO::sts(store, base, 1, ixxxxx<T>(st3, -cs)); IO::sts(store, base + 1, 1, ixxxxx<T>(st3, cs)); }
+                    else          { IO::sts(store, base, 1, oxxxxx<T>(st3, -cs)); IO::sts(store, base + 1, 1, oxxxxx<T>(st3, cs)); }
+                } else {
+                    // the spinors of the two events are formed one by one (scalar FP32) and zipped: their construction branches on the chirality only
+                    sp2<float> f[2][2];
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        const float st3[3] = {(float)b[j][0], (float)b[j][1], (float)b[j][2]};
+                        const float c1 = ((info >> 8) & 1u) ? 1.f : -1.f;
+                        if (ty == 2u) { f[j][0] = ixxxxx<float>(st3, -c1); f[j][1] = ixxxxx<float>(st3, c1); }
+                        else          { f[j][0] = oxxxxx<float>(st3, -c1); f[j][1] = oxxxxx<float>(st3, c1); }
+                    }
+#pragma unroll
+                    for (int v = 0; v < 2; ++v) {
+                        sp2<T> z;
+                        z.s[0] = mk<T>(EL::pack(f[0][v].s[0].re, f[1][v].s[0].re), EL::pack(f[0][v].s[0].im, f[1][v].s[0].im));
+                        z.s[1] = mk<T>(EL::pack(f[0][v].s[1].re, f[1][v].s[1].re), EL::pack(f[0][v].s[1].im, f[1][v].s[1].im));
+                        IO::sts(store, base + v, 1, z);
+                    }
+                }
             }
         }
     }
@@ -419,7 +480,7 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
                     const uint4 td = __ldg(reinterpret_cast<const uint4*>(d.a_term) + (size_t)(t0 + t) * 32 + lane);
                     const unsigned kind = (hdr.y >> (4 * t)) & 15u;
                     const unsigned aa = td.x & 0xffffu, ab = td.x >> 16, ac = td.y & 0xffffu, la = (td.y >> 16) & 7u, lb = (td.y >> 19) & 7u, lc = (td.y >> 22) & 7u;
-                    const T coef = __ldg(cf + td.w);
+                    const T coef = cf[td.w];
                     if (kind == 0u) {
                         vacc(acc, jvvxx0<T>(IO::ldv(store, aa, la), IO::ldk(evK, td.z & 0xffu), IO::ldv(store, ab, lb), IO::ldk(evK, (td.z >> 8) & 0xffu), coef, inv));
                     } else if (kind == 1u) {
@@ -436,7 +497,7 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
                 for (int t = 0; t < nt; ++t) {
                     const uint4 td = __ldg(reinterpret_cast<const uint4*>(d.a_term) + (size_t)(t0 + t) * 32 + lane);
                     const unsigned aa = td.x & 0xffffu, ab = td.x >> 16, la = (td.y >> 16) & 7u, lb = (td.y >> 19) & 7u;
-                    const T coef = __ldg(cf + td.w);
+                    const T coef = cf[td.w];
                     const T chi = ((td.y >> 25) & 1u) ? T(1) : T(-1);
                     if (ptype == 1) sacc(acc, fvixx0<T>(IO::lds(store, aa, la), IO::ldv(store, ab, lb), ko, chi, coef, inv));
                     else            sacc(acc, fvoxx0<T>(IO::lds(store, aa, la), IO::ldv(store, ab, lb), ko, chi, coef, inv));
@@ -457,10 +518,17 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     bool chunk_on = true;
     if (hel_mode == 2) { wgt = (hvalid && h == hel_fixed) ? T(1) : T(0); chunk_on = hel_fixed >= wie * d.cpc && hel_fixed < (wie + 1) * d.cpc; }
     else if (hel_mode == 1) {
-        unsigned int r[4]; const unsigned long long ge = first_event + e;
-        philox4x32_10((unsigned int)ge, (unsigned int)(ge >> 32), 0xffffffffu, 0u, (unsigned int)seed, (unsigned int)(seed >> 32), r);
-        const int hx = d.evalidx[r[0] >> (32 - n)];
-        wgt = (hvalid && h == hx) ? T(1 << n) : T(0); chunk_on = hx >= wie * d.cpc && hx < (wie + 1) * d.cpc;
+        double wj[2] = {0.0, 0.0}; chunk_on = false;
+#pragma unroll
+        for (int j = 0; j < EV; ++j) {
+            unsigned int r[4]; unsigned long long ej = e + j; if (ej >= n_events) ej = n_events - 1;
+            const unsigned long long ge = first_event + ej;
+            philox4x32_10((unsigned int)ge, (unsigned int)(ge >> 32), 0xffffffffu, 0u, (unsigned int)seed, (unsigned int)(seed >> 32), r);
+            const int hx = d.evalidx[r[0] >> (32 - n)];
+            wj[j] = (hvalid && h == hx) ? (double)(1 << n) : 0.0;
+            chunk_on = chunk_on || (hx >= wie * d.cpc && hx < (wie + 1) * d.cpc);
+        }
+        wgt = hg::el<T>::pack(wj[0], wj[EV - 1]);
     }
     T form = T(0);
     if (chunk_on) {
@@ -543,9 +611,9 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
                         const float4 c0 = *reinterpret_cast<const float4*>(cblk + q * 8), c1 = *reinterpret_cast<const float4*>(cblk + q * 8 + 4);
                         c8[0] = c0.x; c8[1] = c0.y; c8[2] = c0.z; c8[3] = c0.w; c8[4] = c1.x; c8[5] = c1.y; c8[6] = c1.z; c8[7] = c1.w;
                     } else {
-                        const double2* rp = reinterpret_cast<const double2*>(cblk + q * 8);
-                        const double2 c0 = rp[0], c1 = rp[1], c2 = rp[2], c3 = rp[3];
-                        c8[0] = c0.x; c8[1] = c0.y; c8[2] = c1.x; c8[3] = c1.y; c8[4] = c2.x; c8[5] = c2.y; c8[6] = c3.x; c8[7] = c3.y;
+                        const uint4* rp = reinterpret_cast<const uint4*>(cblk + q * 8);
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) { const uint4 u = rp[i]; c8[2 * i] = hg::el<T>::from_bits(u.x, u.y); c8[2 * i + 1] = hg::el<T>::from_bits(u.z, u.w); }
                     }
 #pragma unroll
                     for (int i = 0; i < 8; ++i) { tr[i] += c8[i] * xr[q]; ti[i] += c8[i] * xi[q]; }
@@ -564,13 +632,17 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     if (lane == 0 && chunk_on) { atomicAdd(&g_tab_timing[0], (unsigned long long)(tt1 - tt0)); atomicAdd(&g_tab_timing[1], (unsigned long long)(tt2 - tt1)); atomicAdd(&g_tab_timing[2], (unsigned long long)(tt3 - tt2)); atomicAdd(&g_tab_timing[3], (unsigned long long)(tt4 - tt3)); atomicAdd(&g_tab_timing[4], 1ull); }
 #endif
     T acc = wgt * form;          // the helicity sum stays in the kernel's own precision (reading A21)
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) red[el * wpe + wie] = (double)acc;
+#pragma unroll
+    for (int j = 0; j < EV; ++j) {
+        typename hg::el<T>::out_t a = hg::el<T>::half(acc, j);
+        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+        if (lane == 0) red[(el * wpe + wie) * EV + j] = (double)a;
+    }
     if constexpr (JM == 1) { tm_wait_ld(); tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
     __syncthreads();
-    if (te == 0 && live) {
-        T s = T(0); for (int w = 0; w < wpe; ++w) s += (T)red[el * wpe + w];
-        me2[e] = (T)(out_scale * (double)s);
+    if (te < EV && e + te < n_events) {
+        typename hg::el<T>::out_t s = 0; for (int w = 0; w < wpe; ++w) s += (typename hg::el<T>::out_t)red[(el * wpe + w) * EV + te];
+        me2[e + te] = (typename hg::el<T>::out_t)(out_scale * (double)s);
     }
     if constexpr (JM == 1) {
         if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tm_base), "r"((unsigned)tm_cols) : "memory");
