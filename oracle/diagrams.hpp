@@ -40,7 +40,6 @@ inline Process parse_process(const std::string& text) {
     std::istringstream in(text);
     std::string tok;
     bool final_state = false;
-    std::map<std::string, int> multiplicity;
     while (in >> tok) {
         if (tok == ">" || tok == "->") { final_state = true; continue; }
         Leg L; L.initial = !final_state; L.anti = false; L.flavour = -1;
@@ -54,14 +53,24 @@ inline Process parse_process(const std::string& text) {
             // arrow enters the diagram at an initial quark or a final antiquark
             L.kind = (L.initial != L.anti) ? LEG_IN : LEG_OUT;
         }
-        if (final_state) multiplicity[tok] += 1;
         P.legs.push_back(L);
     }
     int n_init = 0; for (size_t i = 0; i < P.legs.size(); ++i) n_init += P.legs[i].initial;
     if (n_init != 2 || P.legs.size() < 4 || P.legs.size() > 8) throw std::runtime_error("need 2 -> n, 2 <= n <= 6");
+    // identical-particle factor: the final state is symmetrised over particles that cannot be told apart, i.e.
+    // final legs with the same species (gluon / flavour) AND the same particle-antiparticle nature.  Counted pairwise from the
+    // leg list: every final leg that has m identical final legs BEFORE it contributes 1/(m+1); the product is 1/prod k!.
     P.sym_factor = 1.0;
-    for (std::map<std::string, int>::iterator it = multiplicity.begin(); it != multiplicity.end(); ++it)
-        for (int k = 2; k <= it->second; ++k) P.sym_factor /= (double)k;
+    for (size_t i = 2; i < P.legs.size(); ++i) {
+        int earlier_twins = 0;
+        for (size_t j = 2; j < i; ++j) {
+            const Leg& a = P.legs[i]; const Leg& b = P.legs[j];
+            const bool both_gluons = a.kind == LEG_G && b.kind == LEG_G;
+            const bool same_quark = a.kind != LEG_G && b.kind != LEG_G && a.flavour == b.flavour && a.anti == b.anti;
+            if (both_gluons || same_quark) ++earlier_twins;
+        }
+        P.sym_factor /= (double)(earlier_twins + 1);
+    }
     const double na = (P.legs[0].kind == LEG_G) ? 8.0 : 3.0, nb = (P.legs[1].kind == LEG_G) ? 8.0 : 3.0;
     P.avg_color = 1.0 / (na * nb);
     P.avg_spin = 0.25;
