@@ -53,6 +53,13 @@ typedef enum { HEGET_FP64 = 0, HEGET_FP32 = 1, HEGET_FP32X2 = 2 } heget_precisio
  * all configurations (no compiler needed).  AUTO: TABLE for processes with >= 6 external legs, STRAIGHT below. */
 typedef enum { HEGET_KERNEL_AUTO = 0, HEGET_KERNEL_STRAIGHT = 1, HEGET_KERNEL_TABLE = 2 } heget_kernel_t;
 
+/* Colour stage of the TABLE back end (step a7, eq. 10): how J^+ C J is formed on the accumulated basis.
+ * SYMMETRIC: t_a = C_aa J_a + sum_{b>a} 2 C_ab J_b in register tiles, coefficients streamed as numbers (default).
+ * DISTINCT:  the paper's own scheme (Table 4): only the distinct values of the matrix are stored,
+ *            an index map (one byte per element) says which value sits where.
+ * CHOLESKY:  C = L L^T (rank-revealing: null directions of a semi-definite C drop out), form = |L^T J|^2. */
+typedef enum { HEGET_COLOUR_SYMMETRIC = 0, HEGET_COLOUR_DISTINCT = 1, HEGET_COLOUR_CHOLESKY = 2 } heget_colour_stage_t;
+
 /* helicity treatment of eq. 12.  SUM: all 2^n_ext configurations (the graded mode, reading A8).
  * SAMPLE: one configuration per event drawn from Philox(seed, global event index), weighted by 2^n_ext -- what the paper
  * itself ran.  FIXED: the single configuration given in `hel` (no weight). */
@@ -86,6 +93,8 @@ typedef struct {
     int kernel;                /* back end the next heget_eval_me2 takes: HEGET_KERNEL_STRAIGHT or HEGET_KERNEL_TABLE */
     int events_per_block;
     int n_hel_computed;        /* configurations the kernel actually evaluates: n_hel_eval, or half of it when the TABLE back end folds the sum by parity (|M|^2 is invariant under flipping every helicity; each evaluated configuration counts twice) */
+    int colour_stage;          /* heget_colour_stage_t in use (TABLE back end) */
+    int n_color_distinct;      /* distinct non-zero values of the n_color_accum x n_color_accum matrix the kernel contracts */
     int packed_pairs;          /* TABLE back end, FP32: 1 if two events share a warp on packed f32x2 instructions (FFMA2) */
     int j_in_tmem;             /* TABLE back end: 1 if the warps keep their J in tensor memory (TMEM), 0 = shared memory */
     double flops_per_event_tensor; /* flops of the colour stage executed on the tensor pipe (0: vector pipes)        */
@@ -145,6 +154,9 @@ heget_status_t heget_run_host(heget_process_t* proc, uint64_t seed, uint64_t fir
 /* Choose the kernel back end (see heget_kernel_t).  Builds or loads what the choice needs (HEGET_ECOMPILE /
  * HEGET_EUNSUPPORTED as for heget_process_create; the previous choice stays on failure).  HEGET_FP32X2 handles are STRAIGHT only. */
 heget_status_t heget_set_kernel(heget_process_t* proc, heget_kernel_t kernel);
+
+/* TABLE back end only: choose the colour stage (see heget_colour_stage_t); takes effect at the next heget_eval_me2. */
+heget_status_t heget_set_colour_stage(heget_process_t* proc, heget_colour_stage_t stage);
 
 /* STRAIGHT back end only (TABLE accepts 0 and nothing else).  Choose the kernel variant: `lanes` threads share one event and split its helicity configurations among them.
  * 0 = automatic (FP64: the wide variant, FP32: one event per thread where built, else wide; wide = info.lanes_wide = the largest power of two <= 32 dividing n_hel_eval, so a warp works

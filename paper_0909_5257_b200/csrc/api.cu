@@ -8,6 +8,7 @@
 #include <cstring>
 #include <map>
 #include <mutex>
+#include <set>
 #include <string>
 #include <vector>
 #include <dlfcn.h>
@@ -150,6 +151,7 @@ static int effective_lanes(const heget_process* p);
 struct heget_process {
     const hg::ProcDesc* d;
     heget::TabProgram* tab;
+    int colour_stage;              // HEGET_COLOUR_* (TABLE back end)
     hg::TabDev tdev; bool tab_on_device; std::vector<void*> tab_allocs; int tab_epc; TabShape tab_shape; int tab_elem;
     std::string name, tag;
     int n_legs, kernel_req;        // requested back end: HEGET_KERNEL_AUTO / STRAIGHT / TABLE
@@ -314,19 +316,56 @@ static heget_status_t table_to_device(heget_process* p) {
         d.n_entries = t.n_entries; d.n_rows = t.n_rows;
     }
     if ((st = upload(p, t.evalidx, &d.evalidx)) != HEGET_OK) return st;
+    // colour stage: what the tiles hold (heget_tab.cuh, phase C)
+    std::vector<double> cmat = t.cmat;
+    d.cstage = 0; d.cidx = 0; d.cvals = 0;
+    std::vector<double> cvals; std::vector<unsigned char> cidx;
+    if (p->colour_stage == HEGET_COLOUR_CHOLESKY) {
+        // C = L L^T (C is positive semi-definite; a vanishing pivot means the rest of its column vanishes too): rows of L^T in the tile layout
+        const int R = t.R, Rp = t.Rpad;
+        std::vector<double> L((size_t)R * R, 0.0);
+        for (int j = 0; j < R; ++j) {
+            double dj = t.colour_acc[(size_t)j * R + j];
+            for (int k = 0; k < j; ++k) dj -= L[(size_t)j * R + k] * L[(size_t)j * R + k];
+            if (dj <= 1e-12 * t.colour_acc[(size_t)j * R + j]) continue;       // null direction: column j of L stays zero
+            const double lj = sqrt(dj); L[(size_t)j * R + j] = lj;
+            for (int i = j + 1; i < R; ++i) {
+                double v = t.colour_acc[(size_t)i * R + j];
+                for (int k = 0; k < j; ++k) v -= L[(size_t)i * R + k] * L[(size_t)j * R + k];
+                L[(size_t)i * R + j] = v / lj;
+            }
+        }
+        std::fill(cmat.begin(), cmat.end(), 0.0);
+        for (int tl = 0; tl < Rp / 8; ++tl) for (int b = 0; b < R; ++b) for (int i = 0; i < 8; ++i) { const int a = tl * 8 + i; if (a < R && b >= a) cmat[((size_t)tl * Rp + b) * 8 + i] = L[(size_t)b * R + a]; }
+        d.cstage = 2;
+    } else if (p->colour_stage == HEGET_COLOUR_DISTINCT) {
+        std::map<double, int> index;
+        cidx.assign(cmat.size() + 64, 0);
+        for (size_t i = 0; i < cmat.size(); ++i) {
+            std::map<double, int>::iterator it = index.find(cmat[i]);
+            if (it == index.end()) { const int id = (int)cvals.size(); if (id > 255) return fail(HEGET_EUNSUPPORTED, "process '%s': more than 256 distinct colour coefficients", p->name.c_str()); index[cmat[i]] = id; cvals.push_back(cmat[i]); cidx[i] = (unsigned char)id; }
+            else cidx[i] = (unsigned char)it->second;
+        }
+        if ((st = upload(p, cidx, &d.cidx)) != HEGET_OK) return st;
+        d.cstage = 1;
+    }
     if (p->tab_elem == TE_F64) {
-        const double* c = 0; if ((st = upload(p, t.cmat, &c)) != HEGET_OK) return st; d.cmat = c;
+        const double* c = 0; if ((st = upload(p, cmat, &c)) != HEGET_OK) return st; d.cmat = c;
         if ((st = upload(p, t.coef, &c)) != HEGET_OK) return st; d.coef = c;
+        if (d.cstage == 1) { if ((st = upload(p, cvals, &c)) != HEGET_OK) return st; d.cvals = c; }
     } else if (p->tab_elem == TE_F32) {
-        std::vector<float> cm(t.cmat.begin(), t.cmat.end()), cf(t.coef.begin(), t.coef.end()); const float* c = 0;
+        std::vector<float> cm(cmat.begin(), cmat.end()), cf(t.coef.begin(), t.coef.end()), cv(cvals.begin(), cvals.end()); const float* c = 0;
         if ((st = upload(p, cm, &c)) != HEGET_OK) return st; d.cmat = c;
         if ((st = upload(p, cf, &c)) != HEGET_OK) return st; d.coef = c;
+        if (d.cstage == 1) { if ((st = upload(p, cv, &c)) != HEGET_OK) return st; d.cvals = c; }
     } else {      // both halves of a packed value hold the same coefficient
-        std::vector<float> cm(2 * t.cmat.size()), cf(2 * t.coef.size()); const float* c = 0;
-        for (size_t i = 0; i < t.cmat.size(); ++i) cm[2 * i] = cm[2 * i + 1] = (float)t.cmat[i];
+        std::vector<float> cm(2 * cmat.size()), cf(2 * t.coef.size()), cv(2 * cvals.size()); const float* c = 0;
+        for (size_t i = 0; i < cmat.size(); ++i) cm[2 * i] = cm[2 * i + 1] = (float)cmat[i];
         for (size_t i = 0; i < t.coef.size(); ++i) cf[2 * i] = cf[2 * i + 1] = (float)t.coef[i];
+        for (size_t i = 0; i < cvals.size(); ++i) cv[2 * i] = cv[2 * i + 1] = (float)cvals[i];
         if ((st = upload(p, cm, &c)) != HEGET_OK) return st; d.cmat = c;
         if ((st = upload(p, cf, &c)) != HEGET_OK) return st; d.coef = c;
+        if (d.cstage == 1) { if ((st = upload(p, cv, &c)) != HEGET_OK) return st; d.cvals = c; }
     }
     p->tab_shape = tab_shape_of(d, p->tab_elem);
     if (p->tab_shape.epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
@@ -377,7 +416,7 @@ heget_status_t heget_process_create(const char* process, double sqrt_s_hat, doub
         return fail(HEGET_EUNSUPPORTED, "process '%s' has no gluon whose two helicities could share a packed thread", name.c_str());
     heget_process* p = new (std::nothrow) heget_process();
     if (!p) return fail(HEGET_ENOMEM, "out of host memory");
-    p->d = 0; p->tab = 0; p->tab_on_device = false; p->tab_epc = 0; p->name = name; p->tag = tag; p->n_legs = n_legs;
+    p->d = 0; p->tab = 0; p->tab_on_device = false; p->tab_epc = 0; p->colour_stage = HEGET_COLOUR_SYMMETRIC; p->name = name; p->tag = tag; p->n_legs = n_legs;
     p->kernel_req = prec == HEGET_FP32X2 ? HEGET_KERNEL_STRAIGHT : HEGET_KERNEL_AUTO;
     { int ng = 0; const std::string padded = " " + name + " "; for (size_t q = 0; q + 2 < padded.size(); ++q) if (padded[q] == ' ' && padded[q + 1] == 'g' && padded[q + 2] == ' ') ++ng; p->auto_table = n_legs >= 7 || (n_legs == 6 && ng >= 6); }
     p->prec = (int)prec; p->lanes = 0; p->sqrt_s = sqrt_s_hat; p->alpha_s = alpha_s;
@@ -414,6 +453,14 @@ heget_status_t heget_set_kernel(heget_process_t* p, heget_kernel_t kernel) {
     return st;
 }
 
+heget_status_t heget_set_colour_stage(heget_process_t* p, heget_colour_stage_t stage) {
+    if (!p) return fail(HEGET_EINVAL, "heget_set_colour_stage: NULL handle");
+    if (stage != HEGET_COLOUR_SYMMETRIC && stage != HEGET_COLOUR_DISTINCT && stage != HEGET_COLOUR_CHOLESKY) return fail(HEGET_EINVAL, "heget_set_colour_stage: unknown stage %d", (int)stage);
+    if (effective_kernel(p) != HEGET_KERNEL_TABLE) return fail(HEGET_EUNSUPPORTED, "heget_set_colour_stage: the straight-line kernels carry their colour form as literal code; select the TABLE back end first");
+    if ((int)stage != p->colour_stage) { p->colour_stage = (int)stage; table_free_device(p); }      // the tiles are rebuilt at the next launch
+    return HEGET_OK;
+}
+
 heget_status_t heget_set_lanes(heget_process_t* p, int lanes) {
     if (!p) return fail(HEGET_EINVAL, "heget_set_lanes: NULL handle");
     if (effective_kernel(p) == HEGET_KERNEL_TABLE) {
@@ -446,7 +493,8 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
         d.Rpad = t.Rpad;
         const int elem = tab_elem_of(p->prec);
         const TabShape sh = tab_shape_of(d, elem);
-        o->events_per_block = sh.epc * (elem == TE_F32X2 ? 2 : 1); o->threads_per_block = sh.epc * t.nchunks * 32; o->j_in_tmem = sh.jm; o->packed_pairs = elem == TE_F32X2;
+        o->events_per_block = sh.epc * (elem == TE_F32X2 ? 2 : 1); o->threads_per_block = sh.epc * t.nchunks * 32; o->j_in_tmem = sh.jm; o->packed_pairs = elem == TE_F32X2; o->colour_stage = p->colour_stage;
+        { std::set<long long> dv; for (size_t i = 0; i < t.colour_acc.size(); ++i) if (t.colour_acc[i] != 0.0) dv.insert((long long)llround(t.colour_acc[i] * 1e9)); o->n_color_distinct = (int)dv.size(); }
         if (have_dev) {
             cudaFuncAttributes fa;
             cudaError_t e;

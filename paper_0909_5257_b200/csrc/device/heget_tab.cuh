@@ -37,7 +37,10 @@ struct TabDev {
     const unsigned char* b_ent;  // [n_entries + padding] closing records in the byte layout of this precision (tab_entry_bytes<T>() each; api.cu, table_to_device)
     const unsigned char* lanerows; // [n_rows][nchunks * 32] per-lane bytes: variant of a leg set, or validity | chirality << 1
     const void* coef;            // T[]: pool of rational coefficients
-    const void* cmat;            // T[(Rpad/8) * R * 8]
+    const void* cmat;            // T[(Rpad/8 + 1) * Rpad * 8]: tiles of the colour matrix (cstage 0), of its Cholesky factor (cstage 2)
+    int cstage;                  // colour stage: 0 symmetric form with literal coefficients, 1 distinct-value table + index map (the paper's scheme), 2 Cholesky factor |L^T J|^2
+    const unsigned char* cidx;   // cstage 1: index of every coefficient of cmat in cvals
+    const void* cvals;           // cstage 1: T[<= 256] distinct coefficient values
     const short* evalidx;        // [2^n_ext] helicity bits -> evaluated configuration or -1
 };
 
@@ -578,11 +581,20 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
         const int ntile = d.Rpad / 8;
         constexpr int CB = 64 * sizeof(T);                    // bytes of one coefficient block
         __syncwarp();
+        const int cstage = d.cstage;
+        const T* cvals = reinterpret_cast<const T*>(d.cvals);
         auto fetch = [&](int t, int bb, int buf) {
-            if (lane < CB / 16 && t < ntile) {
-                const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + buf * CB + lane * 16);
-                const unsigned char* src = reinterpret_cast<const unsigned char*>(cm + ((size_t)t * d.Rpad + (size_t)8 * bb) * 8) + lane * 16;
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst), "l"(src));
+            const size_t blk = ((size_t)t * d.Rpad + (size_t)8 * bb) * 8;        // first coefficient of the block
+            if (t < ntile) {
+                if (cstage == 1) {                // 64 one-byte indices
+                    if (lane < 4) {
+                        const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + buf * CB + lane * 16);
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst), "l"(d.cidx + blk + lane * 16));
+                    }
+                } else if (lane < CB / 16) {
+                    const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + buf * CB + lane * 16);
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst), "l"(reinterpret_cast<const unsigned char*>(cm + blk) + lane * 16));
+                }
             }
             asm volatile("cp.async.commit_group;\n" ::);
         };
@@ -604,6 +616,20 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
                 }
                 asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp();
                 const T* cblk = reinterpret_cast<const T*>(ring + buf * CB);
+                if (cstage == 1) {
+                    // the paper's colour stage: only the distinct values of the matrix are stored, an index map says
+                    // which one sits where
+                    const unsigned char* iblk = ring + buf * CB;
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) {
+                        const uint2 ib = *reinterpret_cast<const uint2*>(iblk + q * 8);
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            const T c = cvals[((i < 4 ? ib.x : ib.y) >> (8 * (i & 3))) & 0xffu];
+                            tr[i] += c * xr[q]; ti[i] += c * xi[q];
+                        }
+                    }
+                } else {
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
                     T c8[8];
@@ -618,11 +644,17 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
 #pragma unroll
                     for (int i = 0; i < 8; ++i) { tr[i] += c8[i] * xr[q]; ti[i] += c8[i] * xi[q]; }
                 }
+                }
                 __syncwarp();
                 buf ^= 1;
             }
+            if (cstage == 2) {        // tiles of the Cholesky factor: t_k = sum_{b >= k} L_bk J_b, form = sum_k |t_k|^2
 #pragma unroll
-            for (int i = 0; i < 8; ++i) form += dr[i] * tr[i] + di[i] * ti[i];
+                for (int i = 0; i < 8; ++i) form += tr[i] * tr[i] + ti[i] * ti[i];
+            } else {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) form += dr[i] * tr[i] + di[i] * ti[i];
+            }
         }
         asm volatile("cp.async.wait_all;\n" ::);
     }

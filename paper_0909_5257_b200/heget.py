@@ -19,7 +19,7 @@ HEL_SUM, HEL_SAMPLE, HEL_FIXED = 0, 1, 2
 KERNEL_AUTO, KERNEL_STRAIGHT, KERNEL_TABLE = 0, 1, 2
 
 EXPORTS = ["heget_process_create", "heget_process_info", "heget_color_matrix", "heget_sample_momenta", "heget_eval_me2",
-           "heget_run_host", "heget_set_lanes", "heget_set_kernel", "heget_fma_probe", "heget_destroy", "heget_last_error", "heget_launch_count"]
+           "heget_run_host", "heget_set_lanes", "heget_set_kernel", "heget_set_colour_stage", "heget_fma_probe", "heget_destroy", "heget_last_error", "heget_launch_count"]
 
 
 class HegetError(RuntimeError):
@@ -38,7 +38,7 @@ class Info(C.Structure):
                 ("avg_spin", C.c_double), ("avg_color", C.c_double), ("sym_factor", C.c_double),
                 ("flops_per_event", C.c_double), ("flops_per_helicity", C.c_double),
                 ("regs_per_thread", C.c_int), ("local_bytes_per_thread", C.c_int), ("threads_per_block", C.c_int), ("lanes_wide", C.c_int), ("lanes", C.c_int),
-                ("kernel", C.c_int), ("events_per_block", C.c_int), ("n_hel_computed", C.c_int), ("packed_pairs", C.c_int), ("j_in_tmem", C.c_int), ("flops_per_event_tensor", C.c_double)]
+                ("kernel", C.c_int), ("events_per_block", C.c_int), ("n_hel_computed", C.c_int), ("colour_stage", C.c_int), ("n_color_distinct", C.c_int), ("packed_pairs", C.c_int), ("j_in_tmem", C.c_int), ("flops_per_event_tensor", C.c_double)]
 
 
 _lib = None
@@ -62,6 +62,7 @@ def lib():
         L.heget_run_host.argtypes = [vp, u64, u64, u64, vp, vp, vp, C.c_int, vp, vp, vp]
         L.heget_set_lanes.argtypes = [vp, C.c_int]
         L.heget_set_kernel.argtypes = [vp, C.c_int]
+        L.heget_set_colour_stage.argtypes = [vp, C.c_int]
         L.heget_fma_probe.argtypes = [C.c_int, u64, vp, u64, C.POINTER(C.c_double), vp]
         L.heget_destroy.argtypes = [vp]
         L.heget_destroy.restype = None
@@ -144,6 +145,11 @@ class Process:
     def set_kernel(self, kernel):
         """heget_set_kernel: "auto", "straight" (specialised compiled kernel) or "table" (generic table-driven kernels)."""
         _check(lib().heget_set_kernel(self._h, {"auto": KERNEL_AUTO, "straight": KERNEL_STRAIGHT, "table": KERNEL_TABLE}[kernel]))
+        self.info = self.process_info()
+
+    def set_colour_stage(self, stage):
+        """heget_set_colour_stage: "symmetric", "distinct" (the paper's value table + index map) or "cholesky" (TABLE back end)."""
+        _check(lib().heget_set_colour_stage(self._h, {"symmetric": 0, "distinct": 1, "cholesky": 2}[stage]))
         self.info = self.process_info()
 
     def set_lanes(self, lanes):
