@@ -57,8 +57,11 @@ typedef enum { HEGET_KERNEL_AUTO = 0, HEGET_KERNEL_STRAIGHT = 1, HEGET_KERNEL_TA
  * SYMMETRIC: t_a = C_aa J_a + sum_{b>a} 2 C_ab J_b in register tiles, coefficients streamed as numbers (default).
  * DISTINCT:  the paper's own scheme (Table 4): only the distinct values of the matrix are stored,
  *            an index map (one byte per element) says which value sits where.
- * CHOLESKY:  C = L L^T (rank-revealing: null directions of a semi-definite C drop out), form = |L^T J|^2. */
-typedef enum { HEGET_COLOUR_SYMMETRIC = 0, HEGET_COLOUR_DISTINCT = 1, HEGET_COLOUR_CHOLESKY = 2 } heget_colour_stage_t;
+ * CHOLESKY:  C = L L^T (rank-revealing: null directions of a semi-definite C drop out), form = |L^T J|^2.
+ * TENSOR:    the J vectors of every (event, configuration) go to HBM as rows of X and a second kernel contracts Y = X C on the
+ *            tensor cores (FP32: TF32 mma with a 3-term error-compensated split; FP64: DMMA), then sum_a X_a Y_a per row;
+ *            at most 128 colour elements; HEL_SUM only; the library keeps the J buffer (<= 1 GiB, events go through it in chunks). */
+typedef enum { HEGET_COLOUR_SYMMETRIC = 0, HEGET_COLOUR_DISTINCT = 1, HEGET_COLOUR_CHOLESKY = 2, HEGET_COLOUR_TENSOR = 3 } heget_colour_stage_t;
 
 /* helicity treatment of eq. 12.  SUM: all 2^n_ext configurations (the graded mode, reading A8).
  * SAMPLE: one configuration per event drawn from Philox(seed, global event index), weighted by 2^n_ext -- what the paper

@@ -17,6 +17,7 @@
 #include "../../include/heget.h"
 #include "rambo.cuh"
 #include "device/heget_tab.cuh"
+#include "device/heget_colour_tc.cuh"
 #include "gen/tabprog.hpp"
 
 extern "C" int heget_generate_source(const char* tag, const char* process, const char* out_path, char* msg, int msglen);
@@ -152,6 +153,7 @@ struct heget_process {
     const hg::ProcDesc* d;
     heget::TabProgram* tab;
     int colour_stage;              // HEGET_COLOUR_* (TABLE back end)
+    void* tc_x; void* tc_form; size_t tc_cap_events; const void* tc_cfull;      // tensor-core colour stage: J rows, row forms, capacity in events, full symmetric matrix
     hg::TabDev tdev; bool tab_on_device; std::vector<void*> tab_allocs; int tab_epc; TabShape tab_shape; int tab_elem;
     std::string name, tag;
     int n_legs, kernel_req;        // requested back end: HEGET_KERNEL_AUTO / STRAIGHT / TABLE
@@ -338,6 +340,13 @@ static heget_status_t table_to_device(heget_process* p) {
         std::fill(cmat.begin(), cmat.end(), 0.0);
         for (int tl = 0; tl < Rp / 8; ++tl) for (int b = 0; b < R; ++b) for (int i = 0; i < 8; ++i) { const int a = tl * 8 + i; if (a < R && b >= a) cmat[((size_t)tl * Rp + b) * 8 + i] = L[(size_t)b * R + a]; }
         d.cstage = 2;
+    } else if (p->colour_stage == HEGET_COLOUR_TENSOR) {
+        if (t.Rpad > 8 * hg::TC_MAX_NT) return fail(HEGET_EUNSUPPORTED, "process '%s': the tensor-core colour stage takes at most %d colour elements", p->name.c_str(), 8 * hg::TC_MAX_NT);
+        // the full symmetric matrix, padded with zeros to Rpad x Rpad, in the precision of the contraction
+        const int R = t.R, Rp = t.Rpad;
+        if (p->prec == HEGET_FP64) { std::vector<double> cfull((size_t)Rp * Rp, 0.0); for (int a = 0; a < R; ++a) for (int b = 0; b < R; ++b) cfull[(size_t)a * Rp + b] = t.colour_acc[(size_t)a * R + b]; const double* c = 0; if ((st = upload(p, cfull, &c)) != HEGET_OK) return st; p->tc_cfull = c; }
+        else { std::vector<float> cfull((size_t)Rp * Rp, 0.f); for (int a = 0; a < R; ++a) for (int b = 0; b < R; ++b) cfull[(size_t)a * Rp + b] = (float)t.colour_acc[(size_t)a * R + b]; const float* c = 0; if ((st = upload(p, cfull, &c)) != HEGET_OK) return st; p->tc_cfull = c; }
+        d.cstage = 3;
     } else if (p->colour_stage == HEGET_COLOUR_DISTINCT) {
         std::map<double, int> index;
         cidx.assign(cmat.size() + 64, 0);
@@ -416,7 +425,7 @@ heget_status_t heget_process_create(const char* process, double sqrt_s_hat, doub
         return fail(HEGET_EUNSUPPORTED, "process '%s' has no gluon whose two helicities could share a packed thread", name.c_str());
     heget_process* p = new (std::nothrow) heget_process();
     if (!p) return fail(HEGET_ENOMEM, "out of host memory");
-    p->d = 0; p->tab = 0; p->tab_on_device = false; p->tab_epc = 0; p->colour_stage = HEGET_COLOUR_SYMMETRIC; p->name = name; p->tag = tag; p->n_legs = n_legs;
+    p->d = 0; p->tab = 0; p->tab_on_device = false; p->tab_epc = 0; p->colour_stage = HEGET_COLOUR_SYMMETRIC; p->tc_x = 0; p->tc_form = 0; p->tc_cap_events = 0; p->tc_cfull = 0; p->name = name; p->tag = tag; p->n_legs = n_legs;
     p->kernel_req = prec == HEGET_FP32X2 ? HEGET_KERNEL_STRAIGHT : HEGET_KERNEL_AUTO;
     { int ng = 0; const std::string padded = " " + name + " "; for (size_t q = 0; q + 2 < padded.size(); ++q) if (padded[q] == ' ' && padded[q + 1] == 'g' && padded[q + 2] == ' ') ++ng; p->auto_table = n_legs >= 7 || (n_legs == 6 && ng >= 6); }
     p->prec = (int)prec; p->lanes = 0; p->sqrt_s = sqrt_s_hat; p->alpha_s = alpha_s;
@@ -437,6 +446,8 @@ void heget_destroy(heget_process_t* p) {
     if (p->s_mom) cudaFree(p->s_mom);
     if (p->s_w) cudaFree(p->s_w);
     if (p->s_me2) cudaFree(p->s_me2);
+    if (p->tc_x) cudaFree(p->tc_x);
+    if (p->tc_form) cudaFree(p->tc_form);
     table_free_device(p);
     delete p->tab;
     delete p;
@@ -455,7 +466,7 @@ heget_status_t heget_set_kernel(heget_process_t* p, heget_kernel_t kernel) {
 
 heget_status_t heget_set_colour_stage(heget_process_t* p, heget_colour_stage_t stage) {
     if (!p) return fail(HEGET_EINVAL, "heget_set_colour_stage: NULL handle");
-    if (stage != HEGET_COLOUR_SYMMETRIC && stage != HEGET_COLOUR_DISTINCT && stage != HEGET_COLOUR_CHOLESKY) return fail(HEGET_EINVAL, "heget_set_colour_stage: unknown stage %d", (int)stage);
+    if (stage != HEGET_COLOUR_SYMMETRIC && stage != HEGET_COLOUR_DISTINCT && stage != HEGET_COLOUR_CHOLESKY && stage != HEGET_COLOUR_TENSOR) return fail(HEGET_EINVAL, "heget_set_colour_stage: unknown stage %d", (int)stage);
     if (effective_kernel(p) != HEGET_KERNEL_TABLE) return fail(HEGET_EUNSUPPORTED, "heget_set_colour_stage: the straight-line kernels carry their colour form as literal code; select the TABLE back end first");
     if ((int)stage != p->colour_stage) { p->colour_stage = (int)stage; table_free_device(p); }      // the tiles are rebuilt at the next launch
     return HEGET_OK;
@@ -599,16 +610,55 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         const double iss = 1.0 / p->sqrt_s;
         // parity-folded helicity sum: every evaluated configuration stands for itself and its mirror image
         const double oscale = p->out_scale * (mode == HEGET_HEL_SUM ? (double)p->tab->hel_weight : 1.0);
-#define HG_TAB_LAUNCH(TT, OT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)blocks, threads, sh.smem, s>>>(p->tdev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, iss, oscale, (OT*)d_me2, (int)mode, hel_fixed, seed, first_event)
-        if (p->tab_elem == TE_F64) { if (sh.jm) HG_TAB_LAUNCH(double, double, 1); else HG_TAB_LAUNCH(double, double, 0); }
-        else if (p->tab_elem == TE_F32) { if (sh.jm) HG_TAB_LAUNCH(float, float, 1); else HG_TAB_LAUNCH(float, float, 0); }
-        else { if (sh.jm) HG_TAB_LAUNCH(hg::f2, float, 1); else HG_TAB_LAUNCH(hg::f2, float, 0); }
+#define HG_TAB_LAUNCH(TT, OT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)cblocks, threads, sh.smem, s>>>(dev, epc, sh.tm_cols, sh.tm_wcols, d_mom + first, n_events, count, iss, oscale, (OT*)d_me2 + first, (int)mode, hel_fixed, seed, first_event + first)
+        hg::TabDev dev = p->tdev;
+        const bool tensor = dev.cstage == 3;
+        unsigned long long chunk = n_events;
+        const size_t esz = p->prec == HEGET_FP64 ? 8 : 4;
+        const size_t rows_per_event = (size_t)dev.nchunks * 32 * 2;
+        if (tensor) {
+            if (mode != HEGET_HEL_SUM) return fail(HEGET_EUNSUPPORTED, "heget_eval_me2: the tensor-core colour stage serves HEL_SUM only");
+            // J rows go through HBM in chunks of at most 1 GiB
+            const size_t per_event = rows_per_event * dev.Rpad * esz;
+            chunk = std::max<unsigned long long>(evpc, std::min<unsigned long long>(n_events, ((size_t)1 << 30) / per_event / evpc * evpc));
+            if (p->tc_cap_events < chunk) {
+                if (p->tc_x) cudaFree(p->tc_x); if (p->tc_form) cudaFree(p->tc_form);
+                p->tc_x = 0; p->tc_form = 0; p->tc_cap_events = 0;
+                if (cudaMalloc(&p->tc_x, chunk * per_event) != cudaSuccess || cudaMalloc(&p->tc_form, chunk * rows_per_event * esz) != cudaSuccess) { cudaGetLastError(); return fail(HEGET_ENOMEM, "heget_eval_me2: cannot allocate the J buffer of the tensor-core colour stage"); }
+                p->tc_cap_events = chunk;
+            }
+            dev.jout = p->tc_x;
+        }
+        for (unsigned long long first = 0; first < n_events; first += chunk) {
+            const unsigned long long count = std::min<unsigned long long>(chunk, n_events - first);
+            const unsigned long long cblocks = (count + evpc - 1) / evpc;
+            if (p->tab_elem == TE_F64) { if (sh.jm) HG_TAB_LAUNCH(double, double, 1); else HG_TAB_LAUNCH(double, double, 0); }
+            else if (p->tab_elem == TE_F32) { if (sh.jm) HG_TAB_LAUNCH(float, float, 1); else HG_TAB_LAUNCH(float, float, 0); }
+            else { if (sh.jm) HG_TAB_LAUNCH(hg::f2, float, 1); else HG_TAB_LAUNCH(hg::f2, float, 0); }
+            CU(cudaGetLastError());
+            g_launches++;
+            if (tensor) {
+                const unsigned long long rows = count * rows_per_event;
+                if (p->prec == HEGET_FP64) {
+                    const size_t smem = (size_t)dev.Rpad * (dev.Rpad + 4) * 8;
+                    CU(cudaFuncSetAttribute(hg::k_colour_dmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    hg::k_colour_dmma<<<(unsigned int)((rows + 63) / 64), 256, smem, s>>>((const double*)p->tc_x, (const double*)p->tc_cfull, (double*)p->tc_form, rows, dev.Rpad);
+                    hg::k_colour_finish<double><<<(unsigned int)((count + 7) / 8), 256, 0, s>>>((const double*)p->tc_form, (double*)d_me2 + first, count, (int)rows_per_event, oscale);
+                } else {
+                    const size_t smem = (size_t)2 * dev.Rpad * (dev.Rpad + 8) * 4;
+                    CU(cudaFuncSetAttribute(hg::k_colour_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    hg::k_colour_tf32<<<(unsigned int)((rows + 127) / 128), 256, smem, s>>>((const float*)p->tc_x, (const float*)p->tc_cfull, (float*)p->tc_form, rows, dev.Rpad);
+                    hg::k_colour_finish<float><<<(unsigned int)((count + 7) / 8), 256, 0, s>>>((const float*)p->tc_form, (float*)d_me2 + first, count, (int)rows_per_event, oscale);
+                }
+                CU(cudaGetLastError());
+                g_launches += 2;
+            }
+        }
 #undef HG_TAB_LAUNCH
-        CU(cudaGetLastError());
-        g_launches++;
         return HEGET_OK;
     }
     const hg::ProcDesc* d = p->d;
+
     hg::LaunchArgs a;
     a.d_mom = d_mom; a.n_events = n_events; a.inv_sqrt_s = 1.0 / p->sqrt_s; a.out_scale = p->out_scale; a.d_me2 = d_me2;
     a.hel_mode = (int)mode; a.hel_fixed = hel_fixed; a.seed = seed; a.first_event = first_event; a.lanes = effective_lanes(p);

@@ -38,7 +38,8 @@ struct TabDev {
     const unsigned char* lanerows; // [n_rows][nchunks * 32] per-lane bytes: variant of a leg set, or validity | chirality << 1
     const void* coef;            // T[]: pool of rational coefficients
     const void* cmat;            // T[(Rpad/8 + 1) * Rpad * 8]: tiles of the colour matrix (cstage 0), of its Cholesky factor (cstage 2)
-    int cstage;                  // colour stage: 0 symmetric form with literal coefficients, 1 distinct-value table + index map (the paper's scheme), 2 Cholesky factor |L^T J|^2
+    int cstage;                  // colour stage: 0 symmetric form with literal coefficients, 1 distinct-value table + index map (the paper's scheme), 2 Cholesky factor |L^T J|^2, 3 J handed to the tensor-core kernel
+    void* jout;                  // cstage 3: rows of J written to HBM for the tensor-core contraction (heget_colour_tc.cuh): out_t[(event * nchunks * 32 + configuration) * 2 + re/im][Rpad]
     const unsigned char* cidx;   // cstage 1: index of every coefficient of cmat in cvals
     const void* cvals;           // cstage 1: T[<= 256] distinct coefficient values
     const short* evalidx;        // [2^n_ext] helicity bits -> evaluated configuration or -1
@@ -344,7 +345,7 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_finish(co
 
 // JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp)
 template <typename T, int JM>
-__global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long n_events,
+__global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
         const double inv_sqrt_s, const double out_scale, typename el<T>::out_t* __restrict__ me2, const int hel_mode, const int hel_fixed,
         const unsigned long long seed, const unsigned long long first_event) {
     typedef tabio<T> IO;
@@ -392,7 +393,7 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     const int epe = epc * EV;
     for (int c = tid; c < 4 * n * epe; c += blockDim.x) {
         unsigned long long ee = e0 + (unsigned long long)(c % epe); if (ee >= n_events) ee = n_events - 1;
-        pm[c] = mom[(size_t)(c / epe) * n_events + ee] * inv_sqrt_s;
+        pm[c] = mom[(size_t)(c / epe) * mom_stride + ee] * inv_sqrt_s;
     }
     __syncthreads();
     if constexpr (JM == 1) {
@@ -579,6 +580,22 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
         // (free after phase B) by cp.async, one block ahead, so the latency of the matrix (L2) is hidden.
         const T* cm = reinterpret_cast<const T*>(d.cmat);
         const int ntile = d.Rpad / 8;
+        if (d.cstage == 3) {
+            // hand J to the tensor-core colour kernel: one row per (event, configuration, re/im), Rpad columns, written 8 at a time
+            typedef typename hg::el<T>::out_t OT;
+            OT* X = reinterpret_cast<OT*>(d.jout);
+            for (int bb = 0; bb < ntile; ++bb) {
+                T xr[8], xi[8];
+                jp.block8(8 * bb, R, xr, xi);
+#pragma unroll
+                for (int j = 0; j < EV; ++j) {
+                    if (e + j >= n_events) continue;
+                    OT* row = X + ((((size_t)(e + j) * wpe + wie) * 32 + lane) * 2) * d.Rpad + 8 * bb;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) { row[i] = hg::el<T>::half(xr[i], j); row[d.Rpad + i] = hg::el<T>::half(xi[i], j); }
+                }
+            }
+        } else {
         constexpr int CB = 64 * sizeof(T);                    // bytes of one coefficient block
         __syncwarp();
         const int cstage = d.cstage;
@@ -657,6 +674,7 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
             }
         }
         asm volatile("cp.async.wait_all;\n" ::);
+        }
     }
     // ---- helicity sum (eq. 12) and averaging factors -------------------------------------------------------------
 #ifdef HG_TAB_TIMING      // debug build only: cycles per phase, summed over warps
@@ -672,7 +690,7 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
     }
     if constexpr (JM == 1) { tm_wait_ld(); tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
     __syncthreads();
-    if (te < EV && e + te < n_events) {
+    if (te < EV && e + te < n_events && d.cstage != 3) {
         typename hg::el<T>::out_t s = 0; for (int w = 0; w < wpe; ++w) s += (typename hg::el<T>::out_t)red[(el * wpe + w) * EV + te];
         me2[e + te] = (typename hg::el<T>::out_t)(out_scale * (double)s);
     }

@@ -148,8 +148,8 @@ class Process:
         self.info = self.process_info()
 
     def set_colour_stage(self, stage):
-        """heget_set_colour_stage: "symmetric", "distinct" (the paper's value table + index map) or "cholesky" (TABLE back end)."""
-        _check(lib().heget_set_colour_stage(self._h, {"symmetric": 0, "distinct": 1, "cholesky": 2}[stage]))
+        """heget_set_colour_stage: "symmetric", "distinct" (the paper's value table + index map), "cholesky" or "tensor" (tensor-core contraction through HBM); TABLE back end."""
+        _check(lib().heget_set_colour_stage(self._h, {"symmetric": 0, "distinct": 1, "cholesky": 2, "tensor": 3}[stage]))
         self.info = self.process_info()
 
     def set_lanes(self, lanes):

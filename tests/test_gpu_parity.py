@@ -179,18 +179,19 @@ def test_table_kernel_matches_oracle(events, oracle_process, monkeypatch, name, 
         assert rel_err(out, other).max() <= (1e-11 if precision == "fp64" else 2e-4)
 
 
-@pytest.mark.parametrize("stage", ["distinct", "cholesky"])
+@pytest.mark.parametrize("stage", ["distinct", "cholesky", "tensor"])
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 @pytest.mark.parametrize("name,sqrt_s,seed,n", [c for c in TABLE_CASES if c[0] in ("u u~ > g g g g", "g g > g g g g", "u u~ > g g g g g", "u u > u u g g g", "u u > u u g g")])
 def test_colour_stage_variants(events, oracle_process, name, sqrt_s, seed, n, precision, stage):
     """NEXT-2: the paper's distinct-value table with an index map and the rank-revealing
     Cholesky form |L^T J|^2 give the same colour sum as the symmetric form -- u u -> u u g g g exercises the null directions
-    of a semi-definite colour matrix (48 accumulated elements, rank 46)."""
+    of a semi-definite colour matrix (48 accumulated elements, rank 46).  "tensor" (row a7-TC): the J vectors go through HBM and
+    Y = X C runs on the tensor cores (TF32 with a 3-term split in FP32, DMMA in FP64) -- same tolerances."""
     mom, mom_h = events(name, sqrt_s, seed, n)
     P = hg.Process(name, sqrt_s, precision=precision, kernel="table")
     base = P.eval_me2(mom).cpu().numpy().astype(np.float64)
     P.set_colour_stage(stage)
-    assert P.info.colour_stage == {"distinct": 1, "cholesky": 2}[stage] and P.info.n_color_distinct > 0
+    assert P.info.colour_stage == {"distinct": 1, "cholesky": 2, "tensor": 3}[stage] and P.info.n_color_distinct > 0
     out = P.eval_me2(mom).cpu().numpy().astype(np.float64)
     ref = oracle_process(name).me2(mom_h)
     err = rel_err(out, ref)
