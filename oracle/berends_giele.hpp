@@ -10,7 +10,10 @@
 // so that the full amplitude is  sum_sigma Tr(T^{a_s(0)} ... T^{a_s(n-1)}) * A(s(0),...,s(n-1))  over
 // non-cyclic orderings -- the expansion of eq. 8 / eq. 17.
 #pragma once
+#include <algorithm>
+#include <vector>
 #include "kin.hpp"
+#include "su3.hpp"
 
 namespace orc {
 
@@ -59,5 +62,45 @@ inline cplx bg_partial_amplitude(int n, const double (*p)[4], const int* hel, co
             for (int m = 0; m < 4; ++m) J[i][j].v[m] = cplx(0.0, -0.5) * acc.v[m] / K2;
         }
     return mdot(eps[n - 1], V[0][n - 2]);
+}
+
+// Tier O1 colour definition on tier O3 kinematics, for pure-gluon processes too large for diagrams.hpp / colour.hpp (g g -> 5 g:
+// 7245 diagrams, 720 traces): the colour-summed squared amplitude of ONE helicity configuration,
+//     sum over all 8^n colour assignments {c_i} of | sum_sigma Tr(T^{c_s(0)} ... T^{c_s(n-1)}) A(s(0), ..., s(n-1)) |^2
+// (eq. 8 with the single-trace basis of eq. 17), sigma over the (n-1)! non-cyclic orderings with leg 0 first,
+// A from the recursion above, the traces multiplied out with the numeric Gell-Mann matrices.  The orderings are walked in
+// lexicographic order and the products T^{c_0} T^{c_s(1)} ... are kept as a stack of prefixes, so a step to the next ordering
+// re-multiplies only the tail that changed (plain arithmetic, nothing skipped).
+inline double gluon_colour_sum_bg(int n, const double (*p)[4], const int* hel, double g) {
+    std::vector<int> rest(n - 1); for (int i = 0; i < n - 1; ++i) rest[i] = i + 1;
+    std::vector<std::vector<int> > orders; std::vector<cplx> amp;
+    do {
+        std::vector<int> o(n); o[0] = 0; for (int i = 0; i < n - 1; ++i) o[i + 1] = rest[i];
+        orders.push_back(o); amp.push_back(bg_partial_amplitude(n, p, hel, o.data(), g));
+    } while (std::next_permutation(rest.begin(), rest.end()));
+    const SU3& S = su3();
+    long total = 1; for (int i = 0; i < n; ++i) total *= 8;
+    double sum = 0.0;
+    #pragma omp parallel for schedule(static) reduction(+ : sum)
+    for (long code = 0; code < total; ++code) {
+        int c[16]; long q = code; for (int i = 0; i < n; ++i) { c[i] = (int)(q % 8); q /= 8; }
+        cplx pre[16][3][3];                       // pre[d] = T^{c_0} T^{c_o(1)} ... T^{c_o(d)}
+        for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) pre[0][i][j] = S.T[c[0]][i][j];
+        cplx M = 0.0;
+        for (size_t s = 0; s < orders.size(); ++s) {
+            int d0 = 1;
+            if (s > 0) while (orders[s][d0] == orders[s - 1][d0]) ++d0;
+            for (int d = d0; d < n; ++d) {
+                const cplx (*T)[3] = S.T[c[orders[s][d]]];
+                for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {
+                    cplx v = 0.0; for (int k = 0; k < 3; ++k) v += pre[d - 1][i][k] * T[k][j];
+                    pre[d][i][j] = v;
+                }
+            }
+            M += (pre[n - 1][0][0] + pre[n - 1][1][1] + pre[n - 1][2][2]) * amp[s];
+        }
+        sum += std::norm(M);
+    }
+    return sum;
 }
 }  // namespace orc

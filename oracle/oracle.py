@@ -50,6 +50,8 @@ def lib():
         L.orc_colour_sum_O1.restype = C.c_double
         L.orc_colour_sum_O1.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_bg_gluon.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
+        L.orc_gluon_colour_sum_bg.restype = C.c_double
+        L.orc_gluon_colour_sum_bg.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_double]
         _lib = L
     return _lib
 
@@ -169,6 +171,14 @@ def bg_gluon(p, hel, order, gs):
     out = np.zeros(2)
     lib().orc_bg_gluon(len(o), _ptr(p), _ptr(h), _ptr(o), gs, _ptr(out))
     return out[0] + 1j * out[1]
+
+
+def gluon_colour_sum_bg(p, hel, gs):
+    """sum over all 8^n colour assignments of |sum_sigma Tr(T^{c_sigma}) A_sigma|^2 for one helicity configuration of an n-gluon
+    process, A_sigma from the Berends-Giele recursion (tier O1 colour on tier O3 kinematics; no diagrams, no colour basis)."""
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    h = np.ascontiguousarray(hel, dtype=np.int32)
+    return lib().orc_gluon_colour_sum_bg(p.shape[0], _ptr(p), _ptr(h), gs)
 
 
 def max_threads():

@@ -118,5 +118,9 @@ void orc_bg_gluon(int n, const double* p_aos, const int* hel, const int* order, 
     cplx a = bg_partial_amplitude(n, (const double (*)[4])p_aos, hel, order, gs);
     out[0] = a.real(); out[1] = a.imag();
 }
+// colour-summed squared amplitude of one helicity configuration of an n-gluon process: explicit colour sum over Berends-Giele partial amplitudes
+double orc_gluon_colour_sum_bg(int n, const double* p /* [n][4] */, const int* hel, double gs) {
+    return gluon_colour_sum_bg(n, (const double (*)[4])p, hel, gs);
+}
 
 }  // extern "C"

@@ -179,6 +179,42 @@ def test_table_kernel_matches_oracle(events, oracle_process, monkeypatch, name, 
         assert rel_err(out, other).max() <= (1e-11 if precision == "fp64" else 2e-4)
 
 
+def test_gg_to_5g_against_explicit_colour_sum():
+    """NEXT-4: g g -> g g g g g (7245 diagrams, 720 colours; the paper compiled it in 140 pieces over 90 minutes and could not run
+    it).  The oracle's diagram/colour-basis tier cannot build its colour matrix (8^7 assignments x 720 traces x
+    7245 diagrams), so single helicity configurations are checked against the explicit colour sum over Berends-Giele partial
+    amplitudes (oracle.gluon_colour_sum_bg: literal SU(3) traces, no diagrams; pinned on 5 and 6 gluons against the diagram tier
+    and on 7 gluons against Parke-Taylor in tests/test_oracle_amplitudes.py); plus what holds for the full sum at any size."""
+    name, sqrt_s = "g g > g g g g g", 2000.0
+    P = hg.Process(name, sqrt_s, precision="fp64")
+    i = P.info
+    assert (i.n_diagrams, i.n_color, i.n_color_accum, i.kernel) == (7245, 720, 120, hg.KERNEL_TABLE)
+    n = 300
+    mom = P.sample_momenta(12, n)
+    mom_h = mom.cpu().numpy()
+    gs = math.sqrt(4 * math.pi * 0.118)
+    fac = 0.25 / 64.0 / 120.0                     # 1/4 spins, 1/(8*8) colours, 1/5! identical gluons
+    for hel in ([1, 1, 1, 1, 1, 1, 1], [1, -1, -1, 1, -1, 1, 1]):      # all-outgoing (--+++++): MHV; (-+-+-++): NMHV
+        out = P.eval_me2(mom, mode=hg.HEL_FIXED, hel=hel).cpu().numpy()
+        for e in (0, 299):
+            ref = fac * O.gluon_colour_sum_bg(mom_h[:, :, e].copy(), hel, gs)
+            assert abs(out[e] / ref - 1.0) <= 1e-10, "hel %s event %d: %g vs %g" % (hel, e, out[e], ref)
+    full = P.eval_me2(mom)
+    assert bool(torch.isfinite(full).all()) and float(full.min()) > 0
+    # Bose symmetry of the full sum, and FP32 against FP64
+    sw = mom.clone(); sw[3], sw[5] = mom[5], mom[3]
+    assert ((P.eval_me2(sw) - full).abs() / full).max().item() <= 1e-11
+    P32 = hg.Process(name, sqrt_s, precision="fp32")
+    e32 = ((P32.eval_me2(mom).double() - full).abs() / full).cpu().numpy()
+    assert np.median(e32) <= TOL32_MEDIAN and e32.max() <= TOL32_MAX
+    # the sum of all 128 single configurations is the full sum (parity-folded inside the kernel)
+    head = mom[:, :, :16].contiguous()
+    tot = torch.zeros(16, dtype=torch.float64, device="cuda")
+    for bits in range(128):
+        tot += P.eval_me2(head, mode=hg.HEL_FIXED, hel=[1 if (bits >> q) & 1 else -1 for q in range(7)])
+    assert ((tot - full[:16]).abs() / full[:16]).max().item() <= 1e-11
+
+
 @pytest.mark.parametrize("stage", ["distinct", "cholesky", "tensor"])
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 @pytest.mark.parametrize("name,sqrt_s,seed,n", [c for c in TABLE_CASES if c[0] in ("u u~ > g g g g", "g g > g g g g", "u u~ > g g g g g", "u u > u u g g g", "u u > u u g g")])

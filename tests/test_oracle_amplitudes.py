@@ -262,3 +262,48 @@ def test_berends_giele_cross_check(oracle_process, name):
         for al in range(0, P.n_color, 1 if n < 6 else 7):
             bg = O.bg_gluon(p, hel, P.basis_element(al)[2][0], P.gs)
             assert abs(bg - J[al]) < 1e-10 * max(np.abs(J).max(), P.gs ** (n - 2))
+
+
+@pytest.mark.parametrize("name,sqrt_s", [("g g > g g g", 1000.0), ("g g > g g g g", 1500.0)])
+def test_explicit_colour_sum_over_bg_amplitudes(oracle_process, name, sqrt_s):
+    """gluon_colour_sum_bg (explicit sum over all 8^n colour assignments of traces times Berends-Giele partial amplitudes: no
+    diagrams, no colour matrix) against tier O2 (diagrams + colour basis + brute-force matrix) per helicity configuration.  This
+    pins the routine that validates g g -> 5 g, where tier O2's colour build (8^7 x 720) is out of reach."""
+    P = oracle_process(name)
+    n = P.n_ext
+    mom, _, _ = O.sample_momenta(n - 2, sqrt_s, 4, 2)
+    # physical helicities; the incoming legs 0, 1 flip in the all-outgoing convention: MHV (two negative) and, for n = 6, NMHV
+    hels = {5: [[1, 1, 1, 1, 1], [1, -1, 1, -1, 1]], 6: [[1, 1, 1, 1, 1, 1], [1, -1, -1, 1, -1, 1]]}[n]
+    for e in range(2):
+        p = np.ascontiguousarray(mom[:, :, e])
+        for hel in hels:
+            s2, _, _ = P.amplitudes(p, hel)
+            s1 = O.gluon_colour_sum_bg(p, hel, P.gs)
+            assert s2 > 0 and abs(s1 / s2 - 1.0) < 1e-11
+
+
+def test_parke_taylor_seven_gluons():
+    """Berends-Giele partial amplitudes of g g -> 5 g against Parke-Taylor for an MHV configuration (all-outgoing helicities
+    with exactly two negative): |A_sigma|^2 = 2^n g^(2n-4) s_ij^4 / prod s_{sigma_a sigma_a+1}, and zero when fewer than two
+    helicities differ from the rest."""
+    n, gs = 7, np.sqrt(4 * np.pi * 0.118)
+    mom, _, _ = O.sample_momenta(5, 2000.0, 13, 1)
+    p = np.ascontiguousarray(mom[:, :, 0])
+    k = all_outgoing(p)
+    rng = np.random.default_rng(3)
+    hel_out = np.array([-1, 1, 1, -1, 1, 1, 1])             # all-outgoing helicities: legs 0 and 3 negative
+    hel = hel_out.copy(); hel[:2] *= -1                      # physical helicities of the two incoming gluons are flipped
+    i, j = 0, 3
+    for _ in range(12):
+        order = [0] + list(rng.permutation(np.arange(1, n)))
+        a = O.bg_gluon(p, hel, order, gs)
+        den = 1.0
+        for q in range(n):
+            den *= sij(k, order[q], order[(q + 1) % n])
+        ref = 2.0 ** n * gs ** (2 * n - 4) * sij(k, i, j) ** 4 / abs(den)
+        assert abs(abs(a) ** 2 / ref - 1.0) < 1e-9
+    # all-plus and one-minus (all-outgoing) vanish
+    for hel_out in ([1] * 7, [-1] + [1] * 6):
+        h = np.array(hel_out); h[:2] *= -1
+        a = O.bg_gluon(p, h, list(range(n)), gs)
+        assert abs(a) < 1e-9 * gs ** 5
