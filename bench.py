@@ -127,12 +127,15 @@ def run_reference(a):
 
 
 def measure(hg, torch, name, sqrt_s, E, seed, precision, steps, warmup, world, rank, first, barrier, max_over_ranks, kernel=None,
-            lanes=0, use_graph=True, extras=True):
+            lanes=0, use_graph=True, extras=True, colour_stage=None):
     """One (config, precision): K timed steps of sample + eval on device-resident buffers, the |M|^2 kernel alone, and the
     host-buffer end-to-end arm.  Returns a dict of raw numbers."""
     P = hg.Process(name, sqrt_s, precision=precision, kernel=kernel)
     if lanes:
         P.set_lanes(lanes)
+    if colour_stage:
+        P.set_colour_stage(colour_stage)
+        extras = extras and colour_stage != "tensor"        # the tensor-core stage serves HEL_SUM only
     info = P.info
     ne = info.n_ext
     mom = torch.empty(ne, 4, E, dtype=torch.float64, device="cuda")
@@ -317,7 +320,7 @@ def run_ours(a):
         E = a.events                      # profiling aid only: not BASELINE.json's size, the workload string says so
     first = rank * E                      # weak scaling: rank r evaluates global events [rE, (r+1)E)
     m = measure(hg, torch, name, sqrt_s, E, seed, a.precision, a.steps, a.warmup, world, rank, first, barrier, max_over_ranks,
-                kernel=a.kernel, lanes=a.lanes, use_graph=not a.no_graph)
+                kernel=a.kernel, lanes=a.lanes, use_graph=not a.no_graph, colour_stage=a.colour_stage)
     info = m["info"]
     pk = peaks()
     sm_max = float(pk.get("sm_max_mhz", 1965.0))
@@ -341,7 +344,7 @@ def run_ours(a):
         for cfg in sorted(CONFIGS):
             for prc in ("fp64", "fp32"):
                 cn, cs, cE, cseed = CONFIGS[cfg]
-                if cfg == a.config and prc == a.precision and a.kernel is None and not a.lanes:
+                if cfg == a.config and prc == a.precision and a.kernel is None and not a.lanes and not a.colour_stage:
                     mm = m
                 else:
                     mm = measure(hg, torch, cn, cs, cE, cseed, prc, a.sweep_steps, 3, 1, 0, 0, barrier, max_over_ranks, extras=False)
@@ -386,6 +389,7 @@ def run_ours(a):
                      "peak_kind": "nominal %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md)" % (SM_COUNT, FP64_LANES if a.precision == "fp64" else FP32_LANES, sm_max),
                      "fma_probe_tflops": probe, "frac_of_probe": roof["achieved"] / probe,
                      "flops_per_event": info.flops_per_event, "executed_flops_per_event": roof["executed_flops_per_event"],
+                     "colour_stage": ["symmetric", "distinct", "cholesky", "tensor"][info.colour_stage] if info.kernel == 2 else "literal code",
                      "kernel_ms": m["kernel_ms"], "sampling_kernel_ms": m["sampling_ms"],
                      "kernel_share_of_step": m["kernel_ms"] / m["ms_per_step"]},
         "cpu_baseline": cpu,
@@ -413,6 +417,7 @@ def main():
     ap.add_argument("--no-graph", action="store_true", help="do not replay small-batch steps from a CUDA graph")
     ap.add_argument("--lanes", type=int, default=0, help="kernel variant (heget_set_lanes); 0 = automatic")
     ap.add_argument("--kernel", default=None, choices=["auto", "straight", "table"], help="kernel back end (heget_set_kernel); default automatic")
+    ap.add_argument("--colour-stage", default=None, choices=["symmetric", "distinct", "cholesky", "tensor"], help="colour stage of the table back end (heget_set_colour_stage)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the per_config table (every config x precision, a few steps each)")
     ap.add_argument("--sweep-steps", type=int, default=3)
     ap.add_argument("--events", type=int, default=0, help="override the events per step (ncu captures of the big configs)")

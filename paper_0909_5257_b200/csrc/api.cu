@@ -210,15 +210,17 @@ template <typename V> static heget_status_t upload(heget_process* p, const std::
 // Launch shape of the table kernels: events per CTA and where J lives (shared memory, or tensor memory = TMEM), chosen for the
 // most resident warps per SM.  Bounds: shared memory, registers (regs per thread of the compiled kernel, 0 = unknown), 2048
 // threads, and for TMEM the 512 columns of an SM (a CTA allocates a power of two >= 32; the warps of a CTA that share a
-// 32-lane quadrant split the columns).  HEGET_TAB_J=smem|tmem forces the choice (experiments).
+// 32-lane quadrant split the columns).  HEGET_TAB_J=smem|tmem and HEGET_TAB_EPC=n force the choice (experiments).
 template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, int regs_smem, int regs_tmem) {
     TabShape best; best.epc = 0; best.jm = 0; best.tm_cols = 0; best.tm_wcols = 0; best.smem = 0; best.warps = -1;
     const char* force = getenv("HEGET_TAB_J");
+    const char* force_epc = getenv("HEGET_TAB_EPC");       // slots per CTA (experiments: the block-size scan of PAPER.md:407)
     for (int jm = 0; jm < 2; ++jm) {
         if (force && ((jm == 0) != (strcmp(force, "smem") == 0))) continue;
         const int regs = jm ? regs_tmem : regs_smem;
         const long reg_warps = regs > 0 ? 65536 / (((regs + 7) / 8 * 8) * 32) : 64;
         for (int epc = 1; epc <= 8; ++epc) {
+            if (force_epc && atoi(force_epc) != epc) continue;
             const int w = epc * d.nchunks, threads = w * 32;
             if (threads > 256) break;
             const size_t smem = hg::tab_smem_bytes<T>(d, epc, jm == 1) + 48;

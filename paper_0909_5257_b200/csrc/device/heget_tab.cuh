@@ -273,15 +273,19 @@ template <typename T> struct JTmem {       // 8-byte elements: 4 columns per com
     unsigned ta;      // TMEM address of column 0 of this warp's block (lane field = first lane of the warp's quadrant)
     __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st4(ta + 4 * k, 0u, 0u, 0u, 0u); tm_wait_st(); }
     __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
-        unsigned r[4][4];
         tm_wait_st();
 #pragma unroll
-        for (int j = 0; j < 4; ++j) if (j < nu) tm_ld4(ta + (off[j] >> 7), r[j][0], r[j][1], r[j][2], r[j][3]);
-        tm_wait_ld();
+        for (int j0 = 0; j0 < 4; j0 += 2) {          // two updates in flight (8 registers) keep the kernel inside its register budget
+            if (j0 >= nu) break;
+            unsigned r[2][4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) if (j < nu) {
-            const T re = el<T>::from_bits(r[j][0], r[j][1]) + c[j] * Sr, im = el<T>::from_bits(r[j][2], r[j][3]) + c[j] * Si;
-            tm_st4(ta + (off[j] >> 7), el<T>::lo(re), el<T>::hi(re), el<T>::lo(im), el<T>::hi(im));
+            for (int j = 0; j < 2; ++j) if (j0 + j < nu) tm_ld4(ta + (off[j0 + j] >> 7), r[j][0], r[j][1], r[j][2], r[j][3]);
+            tm_wait_ld();
+#pragma unroll
+            for (int j = 0; j < 2; ++j) if (j0 + j < nu) {
+                const T re = el<T>::from_bits(r[j][0], r[j][1]) + c[j0 + j] * Sr, im = el<T>::from_bits(r[j][2], r[j][3]) + c[j0 + j] * Si;
+                tm_st4(ta + (off[j0 + j] >> 7), el<T>::lo(re), el<T>::hi(re), el<T>::lo(im), el<T>::hi(im));
+            }
         }
     }
     __device__ __forceinline__ void block8(int k0, int, T* xr, T* xi) {
