@@ -289,13 +289,16 @@ template <typename T> struct JTmem {       // 8-byte elements: 4 columns per com
         }
     }
     __device__ __forceinline__ void block8(int k0, int, T* xr, T* xi) {
-        unsigned r[8][4];
         tm_wait_st();
 #pragma unroll
-        for (int i = 0; i < 8; ++i) tm_ld4(ta + 4 * (k0 + i), r[i][0], r[i][1], r[i][2], r[i][3]);
-        tm_wait_ld();
+        for (int h = 0; h < 8; h += 4) {          // four complex numbers (16 registers) in flight
+            unsigned r[4][4];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) { xr[i] = el<T>::from_bits(r[i][0], r[i][1]); xi[i] = el<T>::from_bits(r[i][2], r[i][3]); }
+            for (int i = 0; i < 4; ++i) tm_ld4(ta + 4 * (k0 + h + i), r[i][0], r[i][1], r[i][2], r[i][3]);
+            tm_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { xr[h + i] = el<T>::from_bits(r[i][0], r[i][1]); xi[h + i] = el<T>::from_bits(r[i][2], r[i][3]); }
+        }
     }
 };
 template <> struct JTmem<float> {
@@ -347,9 +350,11 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_finish(co
     if (C.ctl & 4u) { Sr = T(0); Si = T(0); }
 }
 
-// JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp)
+// JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp).
+// At most 256 threads per CTA (api.cu, tab_pick_shape).  Register budget: 136 for the 8-byte element types (at ptxas' default of
+// 128 the FP64/TMEM instantiation spilled 4 bytes), 128 for float -- zero local memory in all six instantiations.
 template <typename T, int JM>
-__global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
+__global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
         const double inv_sqrt_s, const double out_scale, typename el<T>::out_t* __restrict__ me2, const int hel_mode, const int hel_fixed,
         const unsigned long long seed, const unsigned long long first_event) {
     typedef tabio<T> IO;
@@ -435,16 +440,23 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
                 const double p[4] = {pe[(4 * i) * epe + j], pe[(4 * i + 1) * epe + j], pe[(4 * i + 2) * epe + j], pe[(4 * i + 3) * epe + j]};
                 if (ty < 2u) vxxxxx_basis<double>(p, ty == 1u, b[j], b[j] + 3); else ixxxxx_basis<double>(p, b[j]);
             }
+            const unsigned single = (info >> 9) & 3u;      // 0: both helicities are stored (variants 0, 1); 1 / 2: the leg's helicity is -1 / +1 in every evaluated configuration
             if (ty < 2u) {
                 const T rt[3] = {EL::pack(b[0][0], b[J1][0]), EL::pack(b[0][1], b[J1][1]), EL::pack(b[0][2], b[J1][2])};
                 const T qt[3] = {EL::pack(b[0][3], b[J1][3]), EL::pack(b[0][4], b[J1][4]), EL::pack(b[0][5], b[J1][5])};
-                IO::stv(store, base, 1, vxxxxx<T>(rt, qt, T(-1))); IO::stv(store, base + 1, 1, vxxxxx<T>(rt, qt, T(1)));
+                if (single == 0u) { IO::stv(store, base, 1, vxxxxx<T>(rt, qt, T(-1))); IO::stv(store, base + 1, 1, vxxxxx<T>(rt, qt, T(1))); }
+                else IO::stv(store, base, 0, vxxxxx<T>(rt, qt, single == 2u ? T(1) : T(-1)));
             } else {
                 const T cs = ((info >> 8) & 1u) ? T(1) : T(-1);      // chirality = cs * helicity
                 if constexpr (EV == 1) {
                     const T st3[3] = {EL::pack(b[0][0], 0.0), EL::pack(b[0][1], 0.0), EL::pack(b[0][2], 0.0)};
-                    if (ty == 2u) { IO::sts(store, base, 1, ixxxxx<T>(st3, -cs)); IO::sts(store, base + 1, 1, ixxxxx<T>(st3, cs)); }
-                    else          { IO::sts(store, base, 1, oxxxxx<T>(st3, -cs)); IO::sts(store, base + 1, 1, oxxxxx<T>(st3, cs)); }
+                    if (single == 0u) {
+                        if (ty == 2u) { IO::sts(store, base, 1, ixxxxx<T>(st3, -cs)); IO::sts(store, base + 1, 1, ixxxxx<T>(st3, cs)); }
+                        else          { IO::sts(store, base, 1, oxxxxx<T>(st3, -cs)); IO::sts(store, base + 1, 1, oxxxxx<T>(st3, cs)); }
+                    } else {
+                        const T ch = single == 2u ? cs : -cs;
+                        if (ty == 2u) IO::sts(store, base, 0, ixxxxx<T>(st3, ch)); else IO::sts(store, base, 0, oxxxxx<T>(st3, ch));
+                    }
                 } else {
                     // the spinors of the two events are formed one by one (scalar FP32) and zipped: their construction branches on the chirality only
                     sp2<float> f[2][2];
@@ -457,10 +469,11 @@ __global__ void __launch_bounds__(256) k_tab(const TabDev d, const int epc, cons
                     }
 #pragma unroll
                     for (int v = 0; v < 2; ++v) {
+                        if (single != 0u && v != (int)single - 1) continue;
                         sp2<T> z;
                         z.s[0] = mk<T>(EL::pack(f[0][v].s[0].re, f[1][v].s[0].re), EL::pack(f[0][v].s[0].im, f[1][v].s[0].im));
                         z.s[1] = mk<T>(EL::pack(f[0][v].s[1].re, f[1][v].s[1].re), EL::pack(f[0][v].s[1].im, f[1][v].s[1].im));
-                        IO::sts(store, base + v, 1, z);
+                        if (single == 0u) IO::sts(store, base + v, 1, z); else IO::sts(store, base, 0, z);
                     }
                 }
             }

@@ -41,11 +41,15 @@ struct TabBuilder {
     int hel_of_bit(unsigned bits, int leg) const { return ((bits >> leg) & 1u) ? +1 : -1; }
     int chi_of_leg(unsigned bits, int leg) const { return chisign[leg] * hel_of_bit(bits, leg); }
     // helicity bits of every leg behind current c for its variant v (out-ends of completed quark lines follow their in-ends)
+    // Legs whose helicity is the same in every evaluated configuration (leg 0 after parity folding; both ends of the quark line of
+    // u u~ -> n g) select nothing: they are left out of the variant index, which halves the variants of every current that holds them.
+    unsigned constmask = 0, constbits = 0;
+    unsigned vm(const Cur& c) const { return c.varmask & ~constmask; }
     unsigned pattern(const Cur& c, unsigned v) const {
-        unsigned p = deposit(v, c.varmask);
+        unsigned p = deposit(v, vm(c)) | constbits;
         for (size_t q = 0; q < c.pairs.size(); ++q) {
             const int in = c.pairs[q].first, oe = c.pairs[q].second;
-            if ((c.varmask >> oe) & 1u) continue;
+            if (((c.varmask | constmask) >> oe) & 1u) continue;
             const int h = chi_of_leg(p, in) * chisign[oe];
             if (h > 0) p |= 1u << oe; else p &= ~(1u << oe);
         }
@@ -115,7 +119,7 @@ struct TabBuilder {
         const uint32_t id = (uint32_t)P.coef.size(); P.coef.push_back(f.value()); coef_index[key] = id; return id;
     }
 
-    bool fold_parity = true;
+    bool fold_parity = true, const_legs = true;
     void build(const Graph* paper, bool allow_rank_reduction = true) {
         const int n = G.P.n;
         P.name = G.P.name; P.tag = E.tag; P.n_ext = n; P.n_hel = 1 << n;
@@ -132,6 +136,11 @@ struct TabBuilder {
         for (int h = 0; h < E.NH; ++h) if (!fold_parity || E.hel_of(h)[0] < 0) kept.push_back(h);
         if (fold_parity && 2 * (int)kept.size() != E.NH) throw std::runtime_error("helicity configurations are not closed under parity");
         P.NH = (int)kept.size(); P.n_hel_nonzero = E.NH; P.hel_weight = fold_parity ? 2 : 1;
+        {
+            unsigned all1 = (1u << n) - 1u, all0 = (1u << n) - 1u;      // legs at +1 (at -1) in every evaluated configuration
+            for (size_t q = 0; q < kept.size(); ++q) { const std::vector<int> hv = E.hel_of(kept[q]); unsigned b = 0; for (int i = 0; i < n; ++i) if (hv[i] > 0) b |= 1u << i; all1 &= b; all0 &= ~b; }
+            constmask = const_legs ? (all1 | all0) : 0u; constbits = const_legs ? all1 : 0u;
+        }
         P.nchunks = (P.NH + 31) / 32; P.cpc = (P.NH + P.nchunks - 1) / P.nchunks;
         P.n_diagrams = (int)std::lround(G.n_diagrams_paper); P.n_topologies = (int)std::lround(G.n_topologies);
         const Graph& GP = paper ? *paper : G;
@@ -207,7 +216,7 @@ struct TabBuilder {
             const Cur& C = G.cur[c];
             if ((C.kind == CK_LEAF) != (pass == 0)) continue;
             if (!needed[c] && C.kind != CK_LEAF) continue;
-            lognv[c] = popc(C.varmask);
+            lognv[c] = popc(vm(C));
             if (lognv[c] > 5) throw std::runtime_error("a current with more than 32 helicity variants");
             top = (top + (1 << lognv[c]) - 1) & ~((1 << lognv[c]) - 1);      // base aligned to the variant count: the FP64 layout recovers the variant from the low bits
             base32[c] = top; top += (C.ptype == PT_G ? 2 : 1) << lognv[c];
@@ -215,7 +224,8 @@ struct TabBuilder {
             if (C.kind == CK_LEAF) {
                 const Leg& L = G.P.legs[C.leg];
                 const unsigned ty = L.type == LEG_G ? (L.initial ? 1u : 0u) : (C.ptype == PT_F ? 2u : 3u);
-                P.leginfo[C.leg] = ty | ((chisign[C.leg] > 0 ? 1u : 0u) << 8) | ((unsigned)base32[c] << 16);
+                const unsigned single = ((constmask >> C.leg) & 1u) ? (((constbits >> C.leg) & 1u) ? 2u : 1u) : 0u;      // 0: both helicities stored, 1: only -1, 2: only +1
+                P.leginfo[C.leg] = ty | ((chisign[C.leg] > 0 ? 1u : 0u) << 8) | (single << 9) | ((unsigned)base32[c] << 16);
             } else { P.n_currents++; }
         }
         if (top > 65535) throw std::runtime_error("current store exceeds the 16-bit address space of the tables");
@@ -264,7 +274,7 @@ struct TabBuilder {
                             uint32_t addr[3] = {0, 0, 0}, ln[3] = {0, 0, 0}, ks[2] = {0, 0}, chi = 0;
                             for (int j = 0; j < 3; ++j) if (T.ch[j] >= 0) {
                                 const Cur& A = G.cur[T.ch[j]];
-                                addr[j] = (uint32_t)(base32[T.ch[j]] + (int)extract(pat, A.varmask)); ln[j] = (uint32_t)lognv[T.ch[j]];
+                                addr[j] = (uint32_t)(base32[T.ch[j]] + (int)extract(pat, vm(A))); ln[j] = (uint32_t)lognv[T.ch[j]];
                             }
                             if (T.kind == TA_GGG) { ks[0] = (uint32_t)slot_of(G.cur[T.ch[0]].mask); ks[1] = (uint32_t)slot_of(G.cur[T.ch[1]].mask); }
                             int line_leg = -1;
@@ -343,7 +353,7 @@ struct TabBuilder {
             } else if (cl.kind == AK_IOV) { kind = TB_IOV; c[0] = cl.c[1]; c[1] = cl.c[0]; }      // (psi, psibar, gluon)
             else if (cl.kind != AK_VVV) throw std::runtime_error("closing kind without a table form");
             uint32_t b[4] = {0, 0, 0, 0}, ln[4] = {0, 0, 0, 0}, ks[3] = {0, 0, 0}, rows[4] = {0, 0, 0, 0};
-            for (int j = 0; j < 4; ++j) if (c[j] >= 0) { b[j] = (uint32_t)base32[c[j]]; ln[j] = (uint32_t)lognv[c[j]]; rows[j] = (uint32_t)row_of_mask(G.cur[c[j]].varmask); }
+            for (int j = 0; j < 4; ++j) if (c[j] >= 0) { b[j] = (uint32_t)base32[c[j]]; ln[j] = (uint32_t)lognv[c[j]]; rows[j] = (uint32_t)row_of_mask(vm(G.cur[c[j]])); }
             if (kind == TB_VVV) for (int j = 0; j < 3; ++j) { ks[j] = (uint32_t)slot_of(G.cur[c[j]].mask); if (ks[j] > 255) throw std::runtime_error("more than 256 momentum slots"); }
             const uint32_t fr = (uint32_t)row_of_flags(cl.pairs, kind == TB_IOV ? G.cur[c[0]].end_leg : -1);
             const size_t nu = last ? X[g].size() : 0;

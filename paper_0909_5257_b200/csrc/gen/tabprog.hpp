@@ -23,7 +23,7 @@ struct TabProgram {
     double flops_phase_a = 0, flops_per_hel = 0, flops_colour_per_hel = 0, flops_per_event = 0;
     // prologue
     std::vector<uint32_t> kmask;        // [nK] legs of momentum slot s (its momentum is sum of +-p over them, 1/q^2 beside it)
-    std::vector<uint32_t> leginfo;      // [n]  type (0 final gluon, 1 initial gluon, 2 psi, 3 psibar) | chisign bit << 8 | leaf base32 << 16
+    std::vector<uint32_t> leginfo;      // [n]  type (0 final gluon, 1 initial gluon, 2 psi, 3 psibar) | chisign bit << 8 | stored helicities << 9 (0 both, 1 only -1, 2 only +1) | leaf base32 << 16
     // phase A (currents, once per event and variant)
     std::vector<uint32_t> a_hdr;        // [n_bundles][4]: nterms | out type << 8 | first term index << 16 ; kinds (4 bits each) ; level ; 0
     std::vector<uint32_t> a_out;        // [n_bundles][32][2]
