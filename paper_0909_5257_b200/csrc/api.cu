@@ -254,6 +254,7 @@ template <typename T, int JM> static int tab_kernel_regs() {
     if (cudaFuncGetAttributes(&fa, hg::k_tab<T, JM>) != cudaSuccess) { cudaGetLastError(); return 0; }
     return fa.numRegs;
 }
+template <typename T> static TabShape tab_shape_T(const hg::TabDev& d) { return tab_pick_shape<T>(d, tab_kernel_regs<T, 0>(), tab_kernel_regs<T, 1>()); }
 // FP32 handles run the table program on packed f32x2 arithmetic, two events per warp (HEGET_TAB_PACK=0: scalar, one event per warp)
 static int tab_elem_of(int prec) {
     if (prec == HEGET_FP64) return TE_F64;
@@ -261,9 +262,9 @@ static int tab_elem_of(int prec) {
     return (e && e[0] == '0') ? TE_F32 : TE_F32X2;
 }
 static TabShape tab_shape_of(const hg::TabDev& d, int elem) {
-    if (elem == TE_F64) return tab_pick_shape<double>(d, tab_kernel_regs<double, 0>(), tab_kernel_regs<double, 1>());
-    if (elem == TE_F32) return tab_pick_shape<float>(d, tab_kernel_regs<float, 0>(), tab_kernel_regs<float, 1>());
-    return tab_pick_shape<hg::f2>(d, tab_kernel_regs<hg::f2, 0>(), tab_kernel_regs<hg::f2, 1>());
+    if (elem == TE_F64) return tab_shape_T<double>(d);
+    if (elem == TE_F32) return tab_shape_T<float>(d);
+    return tab_shape_T<hg::f2>(d);
 }
 
 static heget_status_t table_to_device(heget_process* p) {
@@ -290,10 +291,10 @@ static heget_status_t table_to_device(heget_process* p) {
         const size_t npad = (size_t)t.n_entries + HG_TAB_RING + 2;
         std::vector<unsigned char> ent(npad * ENT, 0);
         for (size_t k = 0; k < npad; ++k) {
-            uint32_t w[32]; memset(w, 0, sizeof w);
+            uint32_t w[48]; memset(w, 0, sizeof w);
             if (k >= (size_t)t.n_entries) { w[0] = 3u; memcpy(&ent[k * ENT], w, ENT); continue; }      // null record: no amplitude, no update
             const uint32_t* e = &t.b_rec[k * 16];
-            const unsigned kind = e[0] & 3u, reset = (e[0] >> 2) & 1u, nu = (e[0] >> 3) & 7u;
+            const unsigned kind = e[0] & 3u, reset = (e[0] >> 2) & 1u, nu = (e[0] >> 3) & 15u;
             const unsigned base[4] = {e[1] & 0xffffu, e[1] >> 16, e[2] & 0xffffu, e[2] >> 16};
             unsigned row[4], stride[4];
             for (int j = 0; j < 4; ++j) { row[j] = ((e[3] >> (8 * j)) & 0xffu) * (unsigned)LT; stride[j] = 1u << ((e[0] >> (8 + 3 * j)) & 7u); if (scale * base[j] > 0xffffu || row[j] > 0xffffu) return fail(HEGET_EUNSUPPORTED, "process '%s': current store too large for the table format", p->name.c_str()); }
@@ -310,7 +311,7 @@ static heget_status_t table_to_device(heget_process* p) {
                 for (unsigned j = 0; j < nu; ++j) { const double c = t.coef[e[6 + j] >> 16]; w[12 + 4 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 8u; enc8(c, &w[14 + 4 * j]); }
             } else {
                 const float sf = (float)sgn; memcpy(&w[7], &sf, 4);
-                for (unsigned j = 0; j < nu; ++j) { const float c = (float)t.coef[e[6 + j] >> 16]; w[8 + 2 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 4u; memcpy(&w[9 + 2 * j], &c, 4); }
+                for (unsigned j = 0; j < nu; ++j) { const float c = (float)t.coef[e[6 + j] >> 16]; w[8 + 2 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 4u; memcpy(&w[9 + 2 * j], &c, 4); }      // 8 x {offset, coefficient} from byte 32
             }
             memcpy(&ent[k * ENT], w, ENT);
         }
@@ -382,10 +383,10 @@ static heget_status_t table_to_device(heget_process* p) {
     if (p->tab_shape.epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
     p->tab_epc = p->tab_shape.epc;
     const int smem = (int)p->tab_shape.smem;
-#define HG_TAB_ATTR(TT, JMV) CU(cudaFuncSetAttribute(hg::k_tab<TT, JMV>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem))
-    if (p->tab_elem == TE_F64) { if (p->tab_shape.jm) HG_TAB_ATTR(double, 1); else HG_TAB_ATTR(double, 0); }
-    else if (p->tab_elem == TE_F32) { if (p->tab_shape.jm) HG_TAB_ATTR(float, 1); else HG_TAB_ATTR(float, 0); }
-    else { if (p->tab_shape.jm) HG_TAB_ATTR(hg::f2, 1); else HG_TAB_ATTR(hg::f2, 0); }
+#define HG_TAB_ATTR(TT) do { if (p->tab_shape.jm) CU(cudaFuncSetAttribute(hg::k_tab<TT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); else CU(cudaFuncSetAttribute(hg::k_tab<TT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); } while (0)
+    if (p->tab_elem == TE_F64) HG_TAB_ATTR(double);
+    else if (p->tab_elem == TE_F32) HG_TAB_ATTR(float);
+    else HG_TAB_ATTR(hg::f2);
 #undef HG_TAB_ATTR
     p->tab_on_device = true;
     return HEGET_OK;
@@ -511,9 +512,9 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
         if (have_dev) {
             cudaFuncAttributes fa;
             cudaError_t e;
-            if (elem == TE_F64) e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<double, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<double, 0>);
-            else if (elem == TE_F32) e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<float, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<float, 0>);
-            else e = sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<hg::f2, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<hg::f2, 0>);
+#define HG_TAB_FA(TT) (sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<TT, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<TT, 0>))
+            if (elem == TE_F64) e = HG_TAB_FA(double); else if (elem == TE_F32) e = HG_TAB_FA(float); else e = HG_TAB_FA(hg::f2);
+#undef HG_TAB_FA
             if (e == cudaSuccess) { o->regs_per_thread = fa.numRegs; o->local_bytes_per_thread = (int)fa.localSizeBytes; } else cudaGetLastError();
         }
         return HEGET_OK;
@@ -612,7 +613,7 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         const double iss = 1.0 / p->sqrt_s;
         // parity-folded helicity sum: every evaluated configuration stands for itself and its mirror image
         const double oscale = p->out_scale * (mode == HEGET_HEL_SUM ? (double)p->tab->hel_weight : 1.0);
-#define HG_TAB_LAUNCH(TT, OT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)cblocks, threads, sh.smem, s>>>(dev, epc, sh.tm_cols, sh.tm_wcols, d_mom + first, n_events, count, iss, oscale, (OT*)d_me2 + first, (int)mode, hel_fixed, seed, first_event + first)
+#define HG_TAB_LAUNCH2(TT, OT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)cblocks, threads, sh.smem, s>>>(dev, epc, sh.tm_cols, sh.tm_wcols, d_mom + first, n_events, count, iss, oscale, (OT*)d_me2 + first, (int)mode, hel_fixed, seed, first_event + first)
         hg::TabDev dev = p->tdev;
         const bool tensor = dev.cstage == 3;
         unsigned long long chunk = n_events;
@@ -634,9 +635,10 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         for (unsigned long long first = 0; first < n_events; first += chunk) {
             const unsigned long long count = std::min<unsigned long long>(chunk, n_events - first);
             const unsigned long long cblocks = (count + evpc - 1) / evpc;
-            if (p->tab_elem == TE_F64) { if (sh.jm) HG_TAB_LAUNCH(double, double, 1); else HG_TAB_LAUNCH(double, double, 0); }
-            else if (p->tab_elem == TE_F32) { if (sh.jm) HG_TAB_LAUNCH(float, float, 1); else HG_TAB_LAUNCH(float, float, 0); }
-            else { if (sh.jm) HG_TAB_LAUNCH(hg::f2, float, 1); else HG_TAB_LAUNCH(hg::f2, float, 0); }
+#define HG_TAB_LAUNCH(TT, OT) do { if (sh.jm) HG_TAB_LAUNCH2(TT, OT, 1); else HG_TAB_LAUNCH2(TT, OT, 0); } while (0)
+            if (p->tab_elem == TE_F64) HG_TAB_LAUNCH(double, double);
+            else if (p->tab_elem == TE_F32) HG_TAB_LAUNCH(float, float);
+            else HG_TAB_LAUNCH(hg::f2, float);
             CU(cudaGetLastError());
             g_launches++;
             if (tensor) {
@@ -657,6 +659,7 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
             }
         }
 #undef HG_TAB_LAUNCH
+#undef HG_TAB_LAUNCH2
         return HEGET_OK;
     }
     const hg::ProcDesc* d = p->d;

@@ -50,10 +50,12 @@ template <typename T> __host__ __device__ inline size_t tab_event_bytes(int nK, 
     return (size_t)nK * 4 * sizeof(T) + (((size_t)nK * sizeof(T) + 15) / 16) * 16 + (size_t)store32 * 16 * (sizeof(T) / 4);
 }
 template <typename T> __host__ __device__ inline size_t tab_warp_bytes(int R) { return (size_t)2 * R * 32 * sizeof(T); }
-// a closing record is 64 bytes in FP32 (16 words) and 128 bytes in FP64 (112 used); every warp keeps TAB_RING of them in flight.
+// a closing record is 96 bytes for float (8 header words + 8 colour updates of 8 bytes) and 192 bytes for the 8-byte element types
+// (12 header words + 8 updates of 16 bytes); every warp keeps a ring of TAB_RING of them in shared memory.
 // After phase B the ring double-buffers the blocks of the colour matrix (64 coefficients = 256 / 512 bytes each).
-template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { return sizeof(T) == 4 ? 64 : 128; }
-#define HG_TAB_RING 8
+template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { return sizeof(T) == 4 ? 96 : 192; }
+#define HG_TAB_RING 16
+#define HG_TAB_MAXU 8
 template <typename T> __host__ __device__ inline size_t tab_rows_bytes(int n_rows, int nchunks) { return (((size_t)n_rows * nchunks * 32) + 15) / 16 * 16; }
 template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, bool j_in_tmem = false) {
     const int ev = sizeof(T) == 8 && !std::is_same<T, double>::value ? 2 : 1;      // events per slot
@@ -258,10 +260,10 @@ __device__ __forceinline__ void tm_st4(unsigned ta, unsigned a, unsigned b, unsi
 template <typename T> struct JSmem {
     T* J;
     __device__ __forceinline__ void zero(int R) { for (int a = 0; a < 2 * R; ++a) J[a * 32] = T(0); }
-    // J_k += c_j (Sr, Si) for the nu <= 4 updates of a record; off = byte offset of Re J_k in the lane's column
+    // J_k += c_j (Sr, Si) for the nu <= 8 updates of a record; off = byte offset of Re J_k in the lane's column
     __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) if (j < nu) { T* pj = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(J) + off[j]); pj[0] += c[j] * Sr; pj[32] += c[j] * Si; }
+        for (int j = 0; j < HG_TAB_MAXU; ++j) if (j < nu) { T* pj = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(J) + off[j]); pj[0] += c[j] * Sr; pj[32] += c[j] * Si; }
     }
     // 8 consecutive elements starting at k0 (k0 a multiple of 8)
     __device__ __forceinline__ void block8(int k0, int R, T* xr, T* xi) {
@@ -275,7 +277,7 @@ template <typename T> struct JTmem {       // 8-byte elements: 4 columns per com
     __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
         tm_wait_st();
 #pragma unroll
-        for (int j0 = 0; j0 < 4; j0 += 2) {          // two updates in flight (8 registers) keep the kernel inside its register budget
+        for (int j0 = 0; j0 < HG_TAB_MAXU; j0 += 2) {          // two updates in flight (8 registers) keep the kernel inside its register budget
             if (j0 >= nu) break;
             unsigned r[2][4];
 #pragma unroll
@@ -305,13 +307,17 @@ template <> struct JTmem<float> {
     unsigned ta;
     __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st2(ta + 2 * k, 0u, 0u); tm_wait_st(); }
     __device__ __forceinline__ void update(int nu, const unsigned* off, const float* c, float Sr, float Si) {
-        unsigned r[4][2];
         tm_wait_st();
 #pragma unroll
-        for (int j = 0; j < 4; ++j) if (j < nu) tm_ld2(ta + (off[j] >> 7), r[j][0], r[j][1]);
-        tm_wait_ld();
+        for (int j0 = 0; j0 < HG_TAB_MAXU; j0 += 4) {
+            if (j0 >= nu) break;
+            unsigned r[4][2];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) if (j < nu) tm_st2(ta + (off[j] >> 7), __float_as_uint(__uint_as_float(r[j][0]) + c[j] * Sr), __float_as_uint(__uint_as_float(r[j][1]) + c[j] * Si));
+            for (int j = 0; j < 4; ++j) if (j0 + j < nu) tm_ld2(ta + (off[j0 + j] >> 7), r[j][0], r[j][1]);
+            tm_wait_ld();
+#pragma unroll
+            for (int j = 0; j < 4; ++j) if (j0 + j < nu) tm_st2(ta + (off[j0 + j] >> 7), __float_as_uint(__uint_as_float(r[j][0]) + c[j0 + j] * Sr), __float_as_uint(__uint_as_float(r[j][1]) + c[j0 + j] * Si));
+        }
     }
     __device__ __forceinline__ void block8(int k0, int, float* xr, float* xi) {
         unsigned r[8][2];
@@ -324,26 +330,25 @@ template <> struct JTmem<float> {
     }
 };
 
-// amplitude of one closing into its group sum; at the end of a group, J_k += x_gk S_g (eq. 8) on the lane's column
-template <typename T, typename JP> __device__ __forceinline__ void tab_finish(const TabOps<T>& O, const TabCtl<T>& C, const unsigned char* ent, JP& jp, T& Sr, T& Si) {
+// amplitude of one closing (unit couplings; the kind says which vertex function)
+template <typename T> __device__ __forceinline__ cx<T> tab_amp(const TabOps<T>& O, const TabCtl<T>& C) {
     const unsigned kind = C.ctl & 3u;
-    if (kind != 3u) {
-        cx<T> amp;
-        if (kind == 0u) amp = tab_vvv<T>(O);
-        else if (kind == 1u) amp = tab_gggg<T>(O);
-        else amp = tab_iov<T>(O, C.chi ? T(1) : T(-1));
-        Sr += C.sg * amp.re; Si += C.sg * amp.im;
-    }
-    const int nu = (C.ctl >> 3) & 7u;
+    if (kind == 0u) return tab_vvv<T>(O);
+    if (kind == 1u) return tab_gggg<T>(O);
+    return tab_iov<T>(O, C.chi ? T(1) : T(-1));
+}
+// the amplitude goes into its group sum; at the end of a group, J_k += x_gk S_g (eq. 8) on the lane's column
+template <typename T, typename JP> __device__ __forceinline__ void tab_apply(const cx<T>& amp, const TabCtl<T>& C, const unsigned char* ent, JP& jp, T& Sr, T& Si) {
+    if ((C.ctl & 3u) != 3u) { Sr += C.sg * amp.re; Si += C.sg * amp.im; }
+    const int nu = (C.ctl >> 3) & 15u;
     if (nu) {
-        unsigned off[4]; T c[4];
+        unsigned off[HG_TAB_MAXU]; T c[HG_TAB_MAXU];
         if constexpr (sizeof(T) == 4) {
-            const uint4 u0 = *reinterpret_cast<const uint4*>(ent + 32), u1 = *reinterpret_cast<const uint4*>(ent + 48);
-            off[0] = u0.x; c[0] = __uint_as_float(u0.y); off[1] = u0.z; c[1] = __uint_as_float(u0.w);
-            off[2] = u1.x; c[2] = __uint_as_float(u1.y); off[3] = u1.z; c[3] = __uint_as_float(u1.w);
+#pragma unroll
+            for (int j = 0; j < HG_TAB_MAXU; j += 2) { const uint4 u = *reinterpret_cast<const uint4*>(ent + 32 + 8 * j); off[j] = u.x; c[j] = __uint_as_float(u.y); off[j + 1] = u.z; c[j + 1] = __uint_as_float(u.w); }
         } else {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) { const uint4 uu = *reinterpret_cast<const uint4*>(ent + 48 + 16 * j); off[j] = uu.x; c[j] = el<T>::from_bits(uu.z, uu.w); }
+            for (int j = 0; j < HG_TAB_MAXU; ++j) { const uint4 uu = *reinterpret_cast<const uint4*>(ent + 48 + 16 * j); off[j] = uu.x; c[j] = el<T>::from_bits(uu.z, uu.w); }
         }
         jp.update(nu, off, c, Sr, Si);
     }
@@ -561,31 +566,37 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
         const unsigned char* myrows = rows + wie * 32 + lane;
         // the closing records stream through a per-warp ring in shared memory, six records ahead of their use (cp.async), so the
         // latency of the table (L2) never shows
-        auto issue2 = [&](int k) {        // records k and k + 1 (k even) in one group
-            if (lane < 2 * (ENT / 16)) {
-                const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + (k & (NS - 1)) * ENT + lane * 16);
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(dst), "l"(gent + (size_t)k * ENT + lane * 16));
+        // refill: four records per cp.async group whenever fewer than nine are ahead; after the wait every record below
+        // issued - 4 has landed, and the loop never reads beyond issued - 6
+        int issued = 0;
+        auto refill = [&]() {
+            const unsigned char* src = gent + (size_t)issued * ENT;
+            unsigned char* dst = ring + (issued & (NS - 1)) * ENT;
+#pragma unroll
+            for (int q = 0; q < (4 * ENT + 511) / 512; ++q) {
+                const int o = (q * 32 + lane) * 16;
+                if (o < 4 * ENT) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"((unsigned)__cvta_generic_to_shared(dst + o)), "l"(src + o));
             }
             asm volatile("cp.async.commit_group;\n" ::);
+            issued += 4;
         };
-        auto landed = [&]() { asm volatile("cp.async.wait_group 2;\n" ::); __syncwarp(); };
-        const int nent = d.n_entries;
-        static_assert(HG_TAB_RING == 8, "the prefetch distance below assumes a ring of 8 records");
-        issue2(0); issue2(2); issue2(4);                        // the table is padded with NS + 2 null records
-        landed();
-        // One operand set in registers: fetching the next closing's operands while the current one is computed (a second
-        // set, 44 / 80 more registers) was measured slower in both precisions -- more resident warps hide the shared-memory
-        // latency better than a deeper software pipeline (C4 FP64 3.1e6 -> 4.6e6, FP32 5.7e6 -> 6.8e6 events/s).
+        const int nent = d.n_entries;                             // the table is padded with NS null records
+        static_assert(HG_TAB_RING == 16, "the refill logic assumes a ring of 16 records");
+        refill(); refill(); refill();
+        asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp();
+        // One operand set in registers.  Measured and not adopted: fetching the next closing's operands while the current one is
+        // computed (a second register set: C4 FP64 4.6e6 -> 3.1e6 events/s, the registers are worth more as resident warps), and
+        // evaluating two neighbouring closings of one kind together for more instruction-level parallelism (C5 FP64 9.2e5 -> 8.4e5).
         TabOps<T> O0;
         TabCtl<T> C0;
-        for (int k = 0; k < nent; k += 2) {
-            issue2(k + 6); landed();                            // records k and k + 1 are in the ring
-            tab_load_ops<T>(O0, C0, ring + (k & (NS - 1)) * ENT, store, evK, myrows);
-            tab_finish<T>(O0, C0, ring + (k & (NS - 1)) * ENT, jp, Sr, Si);
-            if (k + 1 < nent) {
-                tab_load_ops<T>(O0, C0, ring + ((k + 1) & (NS - 1)) * ENT, store, evK, myrows);
-                tab_finish<T>(O0, C0, ring + ((k + 1) & (NS - 1)) * ENT, jp, Sr, Si);
-            }
+        for (int k = 0; k < nent;) {
+            if (issued - k <= 8) { refill(); asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp(); }
+            const unsigned char* r0 = ring + (k & (NS - 1)) * ENT;
+            tab_load_ops<T>(O0, C0, r0, store, evK, myrows);
+            cx<T> a0 = mk<T>(T(0), T(0));
+            if ((C0.ctl & 3u) != 3u) a0 = tab_amp<T>(O0, C0);
+            tab_apply<T>(a0, C0, r0, jp, Sr, Si);
+            k += 1;
         }
         asm volatile("cp.async.wait_all;\n" ::);
 #ifdef HG_TAB_TIMING

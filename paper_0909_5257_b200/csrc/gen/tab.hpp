@@ -295,10 +295,27 @@ struct TabBuilder {
         }
 
         // ---- phase B: closings in group order -----------------------------------------------------------------------------
+        // Order of the closings: group by group (a group's amplitudes add up in one register pair); groups sorted by their kind
+        // signature and every other group walked backwards, so closings of one vertex kind come in runs (the kernel's uniform
+        // branch on the kind then changes direction rarely).
         std::vector<int> order;
         { std::vector<std::vector<int> > of_group(ng);
+          auto kind_of = [&](int l) { return G.closings[l].kind == AK_VVV ? 0 : G.closings[l].kind == AK_GGGG ? 1 : 2; };
           for (size_t l = 0; l < G.closings.size(); ++l) if (E.group_of[l] >= 0) of_group[E.group_of[l]].push_back((int)l);
-          for (int g = 0; g < ng; ++g) for (size_t k = 0; k < of_group[g].size(); ++k) order.push_back(of_group[g][k]); }
+          std::vector<std::pair<std::vector<int>, int> > sig(ng);
+          for (int g = 0; g < ng; ++g) {
+              std::stable_sort(of_group[g].begin(), of_group[g].end(), [&](int a, int b) { return kind_of(a) < kind_of(b); });
+              for (size_t k = 0; k < of_group[g].size(); ++k) sig[g].first.push_back(kind_of(of_group[g][k]));
+              sig[g].second = g;
+          }
+          std::stable_sort(sig.begin(), sig.end(), [](const std::pair<std::vector<int>, int>& a, const std::pair<std::vector<int>, int>& b) { return a.first < b.first; });
+          group_order.clear();
+          for (int q = 0; q < ng; ++q) {
+              const int g = sig[q].second;
+              if (q & 1) std::reverse(of_group[g].begin(), of_group[g].end());
+              group_order.push_back(g);
+              for (size_t k = 0; k < of_group[g].size(); ++k) order.push_back(of_group[g][k]);
+          } }
         P.n_closings = (int)order.size();
         const int lanes_total = P.nchunks * 32;
         std::vector<unsigned> cfgbits(P.NH, 0);
@@ -336,10 +353,10 @@ struct TabBuilder {
             return id;
         };
         // one 16-word record per closing (kind 0-2) or per overflow block of colour updates (kind 3):
-        //  [0] kind | reset S << 2 | updates << 3 | log2 nv of the 4 operands << 8 (3 bits each)   [1] base a | b << 16   [2] base c | d << 16
+        //  [0] kind | reset S << 2 | updates (0..8) << 3 | log2 nv of the 4 operands << 8 (3 bits each)   [1] base a | b << 16   [2] base c | d << 16
         //  [3] variant rows of a, b, c, d (bytes)   [4] flag row | ka << 8 | kb << 16 | kc << 24   [5] coefficient of the amplitude in its group sum
-        //  [6..9] colour updates: J element | coefficient index << 16
-        const int MAXU = 4;
+        //  [6..13] colour updates: J element | coefficient index << 16
+        const int MAXU = 8;
         double fl_b = 0;
         P.n_entries = 0;
         for (size_t k = 0; k < order.size(); ++k) {
@@ -362,7 +379,7 @@ struct TabBuilder {
                 const size_t take = std::min<size_t>(MAXU, nu - done);
                 const bool reset = last && done + take == nu;
                 uint32_t w[16]; memset(w, 0, sizeof w);
-                w[0] = (part == 0 ? (uint32_t)kind : 3u) | ((reset ? 1u : 0u) << 2) | ((uint32_t)take << 3) | (ln[0] << 8) | (ln[1] << 11) | (ln[2] << 14) | (ln[3] << 17);
+                w[0] = (part == 0 ? (uint32_t)kind : 3u) | ((reset ? 1u : 0u) << 2) | ((uint32_t)take << 3) | (ln[0] << 8) | (ln[1] << 11) | (ln[2] << 14) | (ln[3] << 17);      // updates: 4 bits (0..8)
                 w[1] = b[0] | (b[1] << 16); w[2] = b[2] | (b[3] << 16);
                 w[3] = rows[0] | (rows[1] << 8) | (rows[2] << 16) | (rows[3] << 24);
                 w[4] = fr | (ks[0] << 8) | (ks[1] << 16) | (ks[2] << 24);
@@ -387,6 +404,7 @@ struct TabBuilder {
         P.flops_per_event = P.flops_phase_a + P.NH * P.flops_per_hel;
     }
     std::vector<Frac> cacc;
+    std::vector<int> group_order;
 
 
     // vertex of a current -> table kind with the operands in the order the device function takes them
