@@ -79,6 +79,9 @@ template <> struct el<float> {
 };
 template <> struct el<double> {
     static constexpr int EV = 1; typedef double out_t;
+    typedef double2 v2;                    // one 16-byte chunk = (re, im), loaded as a native vector: no register shuffling
+    static __device__ __forceinline__ double get(double x) { return x; }
+    static __device__ __forceinline__ double put(double x) { return x; }
     static __device__ __forceinline__ double pack(double a, double) { return a; }
     static __device__ __forceinline__ double half(double v, int) { return v; }
     static __device__ __forceinline__ double from_bits(unsigned lo, unsigned hi) { return __hiloint2double((int)hi, (int)lo); }
@@ -87,14 +90,17 @@ template <> struct el<double> {
 };
 template <> struct el<f2> {
     static constexpr int EV = 2; typedef float out_t;
+    typedef ulonglong2 v2;
+    static __device__ __forceinline__ f2 get(unsigned long long x) { f2 r; r.v = x; return r; }
+    static __device__ __forceinline__ unsigned long long put(f2 x) { return x.v; }
     static __device__ __forceinline__ f2 pack(double a, double b) { return f2((float)a, (float)b); }
     static __device__ __forceinline__ float half(f2 v, int j) { return j ? v.hi() : v.lo(); }
     static __device__ __forceinline__ f2 from_bits(unsigned lo, unsigned hi) { f2 r; r.v = ((unsigned long long)hi << 32) | lo; return r; }
     static __device__ __forceinline__ unsigned lo(f2 v) { return (unsigned)v.v; }
     static __device__ __forceinline__ unsigned hi(f2 v) { return (unsigned)(v.v >> 32); }
 };
-template <typename T> __device__ __forceinline__ cx<T> cx_bits(const uint4 u) { return mk<T>(el<T>::from_bits(u.x, u.y), el<T>::from_bits(u.z, u.w)); }
-template <typename T> __device__ __forceinline__ uint4 bits_cx(const cx<T>& c) { return make_uint4(el<T>::lo(c.re), el<T>::hi(c.re), el<T>::lo(c.im), el<T>::hi(c.im)); }
+template <typename T> __device__ __forceinline__ cx<T> cx_ld(const void* p) { const typename el<T>::v2 u = *reinterpret_cast<const typename el<T>::v2*>(p); return mk<T>(el<T>::get(u.x), el<T>::get(u.y)); }
+template <typename T> __device__ __forceinline__ void cx_st(void* p, const cx<T>& c) { typename el<T>::v2 u; u.x = el<T>::put(c.re); u.y = el<T>::put(c.im); *reinterpret_cast<typename el<T>::v2*>(p) = u; }
 
 template <typename T> struct tabio {       // 8-byte elements (double, f2): one complex per 16-byte chunk
     // chunk of (current base32 b, variant v): 2 b + q nv + v; addr = b + v with b a multiple of nv
@@ -102,25 +108,25 @@ template <typename T> struct tabio {       // 8-byte elements (double, f2): one 
     static __device__ __forceinline__ vec4<T> ldv(const unsigned char* st, unsigned addr, unsigned lnv) {
         const uint4* s = reinterpret_cast<const uint4*>(st) + a64(addr, lnv);
         const unsigned nv = 1u << lnv;
-        vec4<T> w; w.v[0] = cx_bits<T>(s[0]); w.v[1] = cx_bits<T>(s[nv]); w.v[2] = cx_bits<T>(s[2 * nv]); w.v[3] = cx_bits<T>(s[3 * nv]); return w;
+        vec4<T> w; w.v[0] = cx_ld<T>(s); w.v[1] = cx_ld<T>(s + nv); w.v[2] = cx_ld<T>(s + 2 * nv); w.v[3] = cx_ld<T>(s + 3 * nv); return w;
     }
     static __device__ __forceinline__ void stv(unsigned char* st, unsigned addr, unsigned lnv, const vec4<T>& w) {
         uint4* s = reinterpret_cast<uint4*>(st) + a64(addr, lnv);
         const unsigned nv = 1u << lnv;
-        s[0] = bits_cx<T>(w.v[0]); s[nv] = bits_cx<T>(w.v[1]); s[2 * nv] = bits_cx<T>(w.v[2]); s[3 * nv] = bits_cx<T>(w.v[3]);
+        cx_st<T>(s, w.v[0]); cx_st<T>(s + nv, w.v[1]); cx_st<T>(s + 2 * nv, w.v[2]); cx_st<T>(s + 3 * nv, w.v[3]);
     }
     static __device__ __forceinline__ sp2<T> lds(const unsigned char* st, unsigned addr, unsigned lnv) {
         const uint4* s = reinterpret_cast<const uint4*>(st) + a64(addr, lnv);
-        sp2<T> f; f.s[0] = cx_bits<T>(s[0]); f.s[1] = cx_bits<T>(s[1u << lnv]); return f;
+        sp2<T> f; f.s[0] = cx_ld<T>(s); f.s[1] = cx_ld<T>(s + (1u << lnv)); return f;
     }
     static __device__ __forceinline__ void sts(unsigned char* st, unsigned addr, unsigned lnv, const sp2<T>& f) {
         uint4* s = reinterpret_cast<uint4*>(st) + a64(addr, lnv);
-        s[0] = bits_cx<T>(f.s[0]); s[1u << lnv] = bits_cx<T>(f.s[1]);
+        cx_st<T>(s, f.s[0]); cx_st<T>(s + (1u << lnv), f.s[1]);
     }
     static __device__ __forceinline__ mom4<T> ldk(const T* evk, unsigned slot) {
         const uint4* s = reinterpret_cast<const uint4*>(evk) + 2 * slot;
-        const uint4 c0 = s[0], c1 = s[1];
-        mom4<T> k; k.p[0] = el<T>::from_bits(c0.x, c0.y); k.p[1] = el<T>::from_bits(c0.z, c0.w); k.p[2] = el<T>::from_bits(c1.x, c1.y); k.p[3] = el<T>::from_bits(c1.z, c1.w); return k;
+        const cx<T> a = cx_ld<T>(s), b = cx_ld<T>(s + 1);
+        mom4<T> k; k.p[0] = a.re; k.p[1] = a.im; k.p[2] = b.re; k.p[3] = b.im; return k;
     }
 };
 template <> struct tabio<float> {
@@ -162,8 +168,8 @@ template <typename T> struct TabOps { cx<T> w[16]; T k[12]; };
 
 template <typename T> __device__ __forceinline__ void tab_ld(cx<T>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp) {      // 8-byte elements
     const uint4* s = reinterpret_cast<const uint4*>(store) + addr;
-    w[0] = cx_bits<T>(s[0]); w[1] = cx_bits<T>(s[stride]);
-    if (ncomp == 4) { w[2] = cx_bits<T>(s[2 * stride]); w[3] = cx_bits<T>(s[3 * stride]); }
+    w[0] = cx_ld<T>(s); w[1] = cx_ld<T>(s + stride);
+    if (ncomp == 4) { w[2] = cx_ld<T>(s + 2 * stride); w[3] = cx_ld<T>(s + 3 * stride); }
 }
 template <> __device__ __forceinline__ void tab_ld<float>(cx<float>* w, const unsigned char* store, unsigned addr, unsigned stride, int ncomp) {
     const float4* s = reinterpret_cast<const float4*>(store) + addr;
@@ -171,8 +177,8 @@ template <> __device__ __forceinline__ void tab_ld<float>(cx<float>* w, const un
     if (ncomp == 4) { const float4 c1 = s[stride]; w[2] = mk<float>(c1.x, c1.y); w[3] = mk<float>(c1.z, c1.w); }
 }
 template <typename T> __device__ __forceinline__ void tab_ldk4(T* k, const T* p) {      // 8-byte elements
-    const uint4 c0 = reinterpret_cast<const uint4*>(p)[0], c1 = reinterpret_cast<const uint4*>(p)[1];
-    k[0] = el<T>::from_bits(c0.x, c0.y); k[1] = el<T>::from_bits(c0.z, c0.w); k[2] = el<T>::from_bits(c1.x, c1.y); k[3] = el<T>::from_bits(c1.z, c1.w);
+    const cx<T> a = cx_ld<T>(p), b = cx_ld<T>(reinterpret_cast<const uint4*>(p) + 1);
+    k[0] = a.re; k[1] = a.im; k[2] = b.re; k[3] = b.im;
 }
 template <> __device__ __forceinline__ void tab_ldk4<float>(float* k, const float* p) { const float4 c = *reinterpret_cast<const float4*>(p); k[0] = c.x; k[1] = c.y; k[2] = c.z; k[3] = c.w; }
 // closing record (uniform, in the warp's ring).  Word 0: kind (0 vvv, 1 gggg, 2 iov, 3 updates only) | reset S << 2 | updates << 3 |
@@ -182,29 +188,6 @@ template <> __device__ __forceinline__ void tab_ldk4<float>(float* k, const floa
 // FP64: words 8-9 = group coefficient, words 12-27 = 4 x {offset, 0, coefficient}
 template <typename T> struct TabCtl { unsigned ctl; T sg; bool chi; };
 
-template <typename T> __device__ __forceinline__ void tab_load_ops(TabOps<T>& O, TabCtl<T>& C, const unsigned char* ent, const unsigned char* store, const T* evK, const unsigned char* myrows) {
-    const uint4 q0 = *reinterpret_cast<const uint4*>(ent), q1 = *reinterpret_cast<const uint4*>(ent + 16);
-    const unsigned kind = q0.x & 3u;
-    C.ctl = q0.x;
-    T sgc;
-    if constexpr (sizeof(T) == 4) sgc = __uint_as_float(q1.w); else { const uint2 sb = *reinterpret_cast<const uint2*>(ent + 32); sgc = el<T>::from_bits(sb.x, sb.y); }
-    const unsigned fb = myrows[q0.x >> 16];
-    C.sg = (fb & 1u) ? sgc : T(0); C.chi = (fb & 2u) != 0u;
-    if (kind == 3u) return;
-    const unsigned aa = (q0.y & 0xffffu) + myrows[q0.w & 0xffffu], ab = (q0.y >> 16) + myrows[q0.w >> 16], ac = (q0.z & 0xffffu) + myrows[q1.x & 0xffffu];
-    const unsigned sa = q1.y & 0xffu, sb = (q1.y >> 8) & 0xffu, sc = (q1.y >> 16) & 0xffu;
-    if (kind == 0u) {
-        tab_ld<T>(O.w, store, aa, sa, 4); tab_ld<T>(O.w + 4, store, ab, sb, 4); tab_ld<T>(O.w + 8, store, ac, sc, 4);
-        const T* ka = reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(evK) + (q1.z & 0xffffu));
-        const T* kb = reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(evK) + (q1.z >> 16));
-        tab_ldk4<T>(O.k, ka); tab_ldk4<T>(O.k + 4, kb);
-    } else if (kind == 1u) {
-        const unsigned ad = (q0.z >> 16) + myrows[q1.x >> 16], sd = q1.y >> 24;
-        tab_ld<T>(O.w, store, aa, sa, 4); tab_ld<T>(O.w + 4, store, ab, sb, 4); tab_ld<T>(O.w + 8, store, ac, sc, 4); tab_ld<T>(O.w + 12, store, ad, sd, 4);
-    } else {
-        tab_ld<T>(O.w, store, aa, sa, 2); tab_ld<T>(O.w + 2, store, ab, sb, 2); tab_ld<T>(O.w + 4, store, ac, sc, 4);
-    }
-}
 template <typename T> __device__ __forceinline__ cx<T> tab_dot(const cx<T>* a, const cx<T>* b) {      // Minkowski product, 2 MUL + 14 FMA
     cx<T> r;
     r.re = a[0].re * b[0].re - a[0].im * b[0].im - a[1].re * b[1].re + a[1].im * b[1].im - a[2].re * b[2].re + a[2].im * b[2].im - a[3].re * b[3].re + a[3].im * b[3].im;
@@ -330,13 +313,6 @@ template <> struct JTmem<float> {
     }
 };
 
-// amplitude of one closing (unit couplings; the kind says which vertex function)
-template <typename T> __device__ __forceinline__ cx<T> tab_amp(const TabOps<T>& O, const TabCtl<T>& C) {
-    const unsigned kind = C.ctl & 3u;
-    if (kind == 0u) return tab_vvv<T>(O);
-    if (kind == 1u) return tab_gggg<T>(O);
-    return tab_iov<T>(O, C.chi ? T(1) : T(-1));
-}
 // the amplitude goes into its group sum; at the end of a group, J_k += x_gk S_g (eq. 8) on the lane's column
 template <typename T, typename JP> __device__ __forceinline__ void tab_apply(const cx<T>& amp, const TabCtl<T>& C, const unsigned char* ent, JP& jp, T& Sr, T& Si) {
     if ((C.ctl & 3u) != 3u) { Sr += C.sg * amp.re; Si += C.sg * amp.im; }
@@ -348,11 +324,43 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_apply(con
             for (int j = 0; j < HG_TAB_MAXU; j += 2) { const uint4 u = *reinterpret_cast<const uint4*>(ent + 32 + 8 * j); off[j] = u.x; c[j] = __uint_as_float(u.y); off[j + 1] = u.z; c[j + 1] = __uint_as_float(u.w); }
         } else {
 #pragma unroll
-            for (int j = 0; j < HG_TAB_MAXU; ++j) { const uint4 uu = *reinterpret_cast<const uint4*>(ent + 48 + 16 * j); off[j] = uu.x; c[j] = el<T>::from_bits(uu.z, uu.w); }
+            for (int j = 0; j < HG_TAB_MAXU; ++j) { off[j] = *reinterpret_cast<const unsigned*>(ent + 48 + 16 * j); c[j] = cx_ld<T>(ent + 48 + 16 * j).im; }
         }
         jp.update(nu, off, c, Sr, Si);
     }
     if (C.ctl & 4u) { Sr = T(0); Si = T(0); }
+}
+
+// One closing record from start to end.  The kind is tested ONCE and each branch loads its own operands, evaluates its vertex and
+// applies the result, so no value has to be moved into common registers where the branches meet (such moves were 12 % of the
+// instructions when the operands went through one shared structure).
+template <typename T, typename JP> __device__ __forceinline__ void tab_record(const unsigned char* ent, const unsigned char* store, const T* evK, const unsigned char* myrows, JP& jp, T& Sr, T& Si) {
+    const uint4 q0 = *reinterpret_cast<const uint4*>(ent), q1 = *reinterpret_cast<const uint4*>(ent + 16);
+    const unsigned kind = q0.x & 3u;
+    TabCtl<T> C; C.ctl = q0.x;
+    T sgc;
+    if constexpr (sizeof(T) == 4) sgc = __uint_as_float(q1.w); else sgc = cx_ld<T>(ent + 32).re;
+    const unsigned fb = myrows[q0.x >> 16];
+    C.sg = (fb & 1u) ? sgc : T(0); C.chi = (fb & 2u) != 0u;
+    if (kind == 3u) { tab_apply<T>(mk<T>(T(0), T(0)), C, ent, jp, Sr, Si); return; }
+    const unsigned aa = (q0.y & 0xffffu) + myrows[q0.w & 0xffffu], ab = (q0.y >> 16) + myrows[q0.w >> 16], ac = (q0.z & 0xffffu) + myrows[q1.x & 0xffffu];
+    const unsigned sa = q1.y & 0xffu, sb = (q1.y >> 8) & 0xffu, sc = (q1.y >> 16) & 0xffu;
+    if (kind == 0u) {
+        TabOps<T> O;
+        tab_ld<T>(O.w, store, aa, sa, 4); tab_ld<T>(O.w + 4, store, ab, sb, 4); tab_ld<T>(O.w + 8, store, ac, sc, 4);
+        tab_ldk4<T>(O.k, reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(evK) + (q1.z & 0xffffu)));
+        tab_ldk4<T>(O.k + 4, reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(evK) + (q1.z >> 16)));
+        tab_apply<T>(tab_vvv<T>(O), C, ent, jp, Sr, Si);
+    } else if (kind == 1u) {
+        TabOps<T> O;
+        const unsigned ad = (q0.z >> 16) + myrows[q1.x >> 16], sd = q1.y >> 24;
+        tab_ld<T>(O.w, store, aa, sa, 4); tab_ld<T>(O.w + 4, store, ab, sb, 4); tab_ld<T>(O.w + 8, store, ac, sc, 4); tab_ld<T>(O.w + 12, store, ad, sd, 4);
+        tab_apply<T>(tab_gggg<T>(O), C, ent, jp, Sr, Si);
+    } else {
+        TabOps<T> O;
+        tab_ld<T>(O.w, store, aa, sa, 2); tab_ld<T>(O.w + 2, store, ab, sb, 2); tab_ld<T>(O.w + 4, store, ac, sc, 4);
+        tab_apply<T>(tab_iov<T>(O, C.chi ? T(1) : T(-1)), C, ent, jp, Sr, Si);
+    }
 }
 
 // JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp).
@@ -584,19 +592,12 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
         static_assert(HG_TAB_RING == 16, "the refill logic assumes a ring of 16 records");
         refill(); refill(); refill();
         asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp();
-        // One operand set in registers.  Measured and not adopted: fetching the next closing's operands while the current one is
+        // One closing at a time, one operand set in registers.  Measured and not adopted: fetching the next closing's operands while the current one is
         // computed (a second register set: C4 FP64 4.6e6 -> 3.1e6 events/s, the registers are worth more as resident warps), and
         // evaluating two neighbouring closings of one kind together for more instruction-level parallelism (C5 FP64 9.2e5 -> 8.4e5).
-        TabOps<T> O0;
-        TabCtl<T> C0;
-        for (int k = 0; k < nent;) {
+        for (int k = 0; k < nent; ++k) {
             if (issued - k <= 8) { refill(); asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp(); }
-            const unsigned char* r0 = ring + (k & (NS - 1)) * ENT;
-            tab_load_ops<T>(O0, C0, r0, store, evK, myrows);
-            cx<T> a0 = mk<T>(T(0), T(0));
-            if ((C0.ctl & 3u) != 3u) a0 = tab_amp<T>(O0, C0);
-            tab_apply<T>(a0, C0, r0, jp, Sr, Si);
-            k += 1;
+            tab_record<T>(ring + (k & (NS - 1)) * ENT, store, evK, myrows, jp, Sr, Si);
         }
         asm volatile("cp.async.wait_all;\n" ::);
 #ifdef HG_TAB_TIMING
@@ -684,7 +685,7 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
                     } else {
                         const uint4* rp = reinterpret_cast<const uint4*>(cblk + q * 8);
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) { const uint4 u = rp[i]; c8[2 * i] = hg::el<T>::from_bits(u.x, u.y); c8[2 * i + 1] = hg::el<T>::from_bits(u.z, u.w); }
+                        for (int i = 0; i < 4; ++i) { const cx<T> u = cx_ld<T>(rp + i); c8[2 * i] = u.re; c8[2 * i + 1] = u.im; }
                     }
 #pragma unroll
                     for (int i = 0; i < 8; ++i) { tr[i] += c8[i] * xr[q]; ti[i] += c8[i] * xi[q]; }
