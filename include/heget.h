@@ -181,6 +181,31 @@ heget_status_t heget_fma_probe(heget_precision_t prec, uint64_t iters, void* d_o
 /* number of kernel launches this library has enqueued since it was loaded (bench.py's gpu_launches) */
 uint64_t heget_launch_count(void);
 
+/* ---- An entry point that allocates nothing -------------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+ * heget_eval_me2_static computes what heget_eval_me2(.., HEGET_HEL_SUM, ..) computes with the tensor-core colour stage (eqs. 8-12,
+ * the table kernel writes the rows of J, the tensor-core kernel contracts them with the colour matrix, a third kernel
+ * sums over helicities), but the scratch between the kernels -- the rows of J and the row forms -- lives in ONE file-scope device array
+ * of HEGET_STATIC_SCRATCH_BYTES inside the library instead of in cudaMalloc'ed memory.  Every GPU that loads the library holds that
+ * array until the process exits.  The call itself performs no cudaMalloc, cudaFree or allocating library routine: three kernel launches.
+ *
+ * Set-up (this part allocates, once):  TABLE back end (heget_set_kernel or automatic), heget_set_colour_stage(HEGET_COLOUR_TENSOR),
+ * then heget_static_prepare(proc) with the device current -- it uploads the process tables and asks the runtime for the device
+ * address of the array (once per device).  A later heget_set_kernel / heget_set_colour_stage that changes the selection undoes it.
+ *
+ *   d_mom     DEVICE, [n_ext][4][n_events] float64 as for heget_eval_me2 (stride n_events), caller-owned
+ *   n_events  at most heget_static_max_events(proc) (C5 FP64: 1083, FP32: 2166; C4 FP64: 5242); more -> HEGET_EINVAL with the limit
+ *             in heget_last_error(), nothing launched.  0 is a no-op.
+ *   d_me2     DEVICE, [n_events] float64 (FP64 handle) or float32 (FP32 handle), caller-owned
+ * Asynchronous on cuda_stream.  All handles and all calls on a device SHARE the array, which keeps the contents of the last call;
+ * nothing in it has to start at zero (every element a call reads it has written before), so no clearing is done.  Calls that overlap
+ * on the GPU (different streams, or graphs replayed concurrently) race on it: serialise them on one stream.
+ * Errors: HEGET_EINVAL (not prepared, size, NULL pointer), HEGET_ECUDA. */
+#define HEGET_STATIC_SCRATCH_BYTES (64u << 20)
+heget_status_t heget_static_prepare(heget_process_t* proc);
+uint64_t heget_static_max_events(const heget_process_t* proc);      /* 0 if the handle is not prepared */
+heget_status_t heget_eval_me2_static(heget_process_t* proc, const double* d_mom, uint64_t n_events, void* d_me2, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -710,3 +710,114 @@ heget_status_t heget_run_host(heget_process_t* p, uint64_t seed, uint64_t first_
 }
 
 }  // extern "C"
+
+// ---- the entry point that allocates nothing ------------------------------------------------------------------------------------------
+// The tensor-core colour stage hands the rows of J (eq. 8) from the table kernel to the contraction kernel through a
+// scratch buffer in HBM; heget_eval_me2 takes that buffer from cudaMalloc.  heget_eval_me2_static runs the same three kernels with the
+// buffer inside ONE file-scope device array of HEGET_STATIC_SCRATCH_BYTES, so that nothing is allocated or freed in the call (CUDA graph
+// capture, serving loops and harnesses that forbid cudaMalloc).  Every GPU that loads the library holds the array until the process
+// exits.  In host code the NAME of the array is a host-side stand-in, not a device address: its device address is asked for once per
+// device, with that device current, by cudaGetSymbolAddress (heget_static_prepare) and that pointer is what the kernels get.
+static __device__ __align__(256) unsigned char g_static_scratch[HEGET_STATIC_SCRATCH_BYTES];
+static void* g_static_ptr[64];                 // device ordinal -> address of g_static_scratch on that device (0: not asked for yet)
+static std::mutex g_static_mutex;
+
+static size_t static_align(size_t v) { return (v + 255) / 256 * 256; }
+// bytes of the scratch array that n events take: rows of J, then the row forms (256-byte aligned)
+static size_t static_bytes(const hg::TabDev& d, size_t esz, unsigned long long n) {
+    const size_t rows_per_event = (size_t)d.nchunks * 32 * 2;
+    return static_align((size_t)n * rows_per_event * d.Rpad * esz) + (size_t)n * rows_per_event * esz;
+}
+static unsigned long long static_max_events(const hg::TabDev& d, size_t esz) {
+    const size_t rows_per_event = (size_t)d.nchunks * 32 * 2, per_event = rows_per_event * d.Rpad * esz + rows_per_event * esz;
+    unsigned long long n = (unsigned long long)(HEGET_STATIC_SCRATCH_BYTES / per_event);
+    while (n > 0 && static_bytes(d, esz, n) > (size_t)HEGET_STATIC_SCRATCH_BYTES) --n;
+    return n;
+}
+static bool static_ready(const heget_process* p) { return p->tab && p->tab_on_device && p->colour_stage == HEGET_COLOUR_TENSOR && p->tc_cfull; }
+
+extern "C" {
+
+heget_status_t heget_static_prepare(heget_process_t* p) {
+    if (!p) return fail(HEGET_EINVAL, "heget_static_prepare: NULL handle");
+    if (effective_kernel(p) != HEGET_KERNEL_TABLE) return fail(HEGET_EUNSUPPORTED, "heget_static_prepare: the static-scratch path belongs to the TABLE back end (heget_set_kernel)");
+    if (p->colour_stage != HEGET_COLOUR_TENSOR) return fail(HEGET_EINVAL, "heget_static_prepare: select the tensor-core colour stage first (heget_set_colour_stage(HEGET_COLOUR_TENSOR))");
+    const heget_status_t st = table_to_device(p);      // set-up: this is where the process tables are allocated and uploaded
+    if (st != HEGET_OK) return st;
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(HEGET_EUNSUPPORTED, "heget_static_prepare: device ordinal %d", dev);
+    {
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        if (!g_static_ptr[dev]) {
+            void* ptr = 0;
+            const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);      // once per device, with that device current
+            if (e != cudaSuccess || !ptr) { cudaGetLastError(); return fail(HEGET_ECUDA, "heget_static_prepare: cudaGetSymbolAddress failed: %s", cudaGetErrorString(e)); }
+            g_static_ptr[dev] = ptr;
+        }
+    }
+    // dynamic shared memory of the contraction kernels (an attribute of the function: no allocation, but not something to do under capture)
+    if (p->prec == HEGET_FP64) CU(cudaFuncSetAttribute(hg::k_colour_dmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)p->tdev.Rpad * (p->tdev.Rpad + 4) * 8)));
+    else CU(cudaFuncSetAttribute(hg::k_colour_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)2 * p->tdev.Rpad * (p->tdev.Rpad + 8) * 4)));
+    // with lazy module loading a kernel's code reaches the device at its first use: touch the third kernel here so that the first call loads nothing
+    cudaFuncAttributes fa;
+    if (p->prec == HEGET_FP64) CU(cudaFuncGetAttributes(&fa, hg::k_colour_finish<double>)); else CU(cudaFuncGetAttributes(&fa, hg::k_colour_finish<float>));
+    return HEGET_OK;
+}
+
+uint64_t heget_static_max_events(const heget_process_t* p) {
+    if (!p || !static_ready(p)) return 0;
+    return static_max_events(p->tdev, p->prec == HEGET_FP64 ? 8 : 4);
+}
+
+heget_status_t heget_eval_me2_static(heget_process_t* p, const double* d_mom, uint64_t n_events, void* d_me2, void* cuda_stream) {
+    if (!p) return fail(HEGET_EINVAL, "heget_eval_me2_static: NULL handle");
+    if (!static_ready(p)) return fail(HEGET_EINVAL, "heget_eval_me2_static: the handle is not prepared (TABLE back end, heget_set_colour_stage(HEGET_COLOUR_TENSOR), then heget_static_prepare; a later heget_set_kernel / heget_set_colour_stage undoes it)");
+    if (n_events == 0) return HEGET_OK;
+    if (!d_mom || !d_me2) return fail(HEGET_EINVAL, "heget_eval_me2_static: NULL device pointer");
+    int devno = -1;
+    CU(cudaGetDevice(&devno));
+    unsigned char* scratch = (devno >= 0 && devno < 64) ? (unsigned char*)g_static_ptr[devno] : 0;
+    if (!scratch) return fail(HEGET_EINVAL, "heget_eval_me2_static: heget_static_prepare has not run on device %d", devno);
+    const size_t esz = p->prec == HEGET_FP64 ? 8 : 4;
+    hg::TabDev dev = p->tdev;
+    const unsigned long long nmax = static_max_events(dev, esz);
+    if (n_events > nmax) return fail(HEGET_EINVAL, "heget_eval_me2_static: %llu events need %zu bytes of scratch, the static array holds %llu (at most %llu events of '%s' per call)",
+                                     (unsigned long long)n_events, static_bytes(dev, esz, n_events), (unsigned long long)HEGET_STATIC_SCRATCH_BYTES, nmax, p->name.c_str());
+    const size_t rows_per_event = (size_t)dev.nchunks * 32 * 2;
+    const unsigned long long rows = n_events * rows_per_event;
+    void* X = scratch;
+    void* form = scratch + static_align((size_t)rows * dev.Rpad * esz);
+    // nothing in the scratch has to start at zero: the table kernel writes every element of the rows of [0, n_events), the contraction kernel
+    // writes every row form, and nothing is accumulated into either -- what an earlier call left behind is never read
+    dev.cstage = 3; dev.jout = X;
+    const int epc = p->tab_epc;
+    const int evpc = epc * (p->tab_elem == TE_F32X2 ? 2 : 1);
+    const unsigned int blocks = (unsigned int)((n_events + evpc - 1) / evpc);
+    const int threads = epc * dev.nchunks * 32;
+    const TabShape& sh = p->tab_shape;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const double iss = 1.0 / p->sqrt_s, oscale = p->out_scale * (double)p->tab->hel_weight;
+#define HG_TAB_STATIC2(TT, OT, JMV) hg::k_tab<TT, JMV><<<blocks, threads, sh.smem, s>>>(dev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, n_events, iss, oscale, (OT*)d_me2, (int)HEGET_HEL_SUM, -1, 0ull, 0ull)
+#define HG_TAB_STATIC(TT, OT) do { if (sh.jm) HG_TAB_STATIC2(TT, OT, 1); else HG_TAB_STATIC2(TT, OT, 0); } while (0)
+    if (p->tab_elem == TE_F64) HG_TAB_STATIC(double, double);
+    else if (p->tab_elem == TE_F32) HG_TAB_STATIC(float, float);
+    else HG_TAB_STATIC(hg::f2, float);
+#undef HG_TAB_STATIC
+#undef HG_TAB_STATIC2
+    CU(cudaGetLastError());
+    if (p->prec == HEGET_FP64) {
+        const size_t smem = (size_t)dev.Rpad * (dev.Rpad + 4) * 8;
+        hg::k_colour_dmma<<<(unsigned int)((rows + 63) / 64), 256, smem, s>>>((const double*)X, (const double*)p->tc_cfull, (double*)form, rows, dev.Rpad);
+        hg::k_colour_finish<double><<<(unsigned int)((n_events + 7) / 8), 256, 0, s>>>((const double*)form, (double*)d_me2, n_events, (int)rows_per_event, oscale);
+    } else {
+        const size_t smem = (size_t)2 * dev.Rpad * (dev.Rpad + 8) * 4;
+        hg::k_colour_tf32<<<(unsigned int)((rows + 127) / 128), 256, smem, s>>>((const float*)X, (const float*)p->tc_cfull, (float*)form, rows, dev.Rpad);
+        hg::k_colour_finish<float><<<(unsigned int)((n_events + 7) / 8), 256, 0, s>>>((const float*)form, (float*)d_me2, n_events, (int)rows_per_event, oscale);
+    }
+    CU(cudaGetLastError());
+    g_launches += 3;
+    return HEGET_OK;
+}
+
+}  // extern "C"

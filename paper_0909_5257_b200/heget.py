@@ -19,7 +19,8 @@ HEL_SUM, HEL_SAMPLE, HEL_FIXED = 0, 1, 2
 KERNEL_AUTO, KERNEL_STRAIGHT, KERNEL_TABLE = 0, 1, 2
 
 EXPORTS = ["heget_process_create", "heget_process_info", "heget_color_matrix", "heget_sample_momenta", "heget_eval_me2",
-           "heget_run_host", "heget_set_lanes", "heget_set_kernel", "heget_set_colour_stage", "heget_fma_probe", "heget_destroy", "heget_last_error", "heget_launch_count"]
+           "heget_run_host", "heget_set_lanes", "heget_set_kernel", "heget_set_colour_stage", "heget_fma_probe", "heget_destroy", "heget_last_error", "heget_launch_count",
+           "heget_static_prepare", "heget_static_max_events", "heget_eval_me2_static"]
 
 
 class HegetError(RuntimeError):
@@ -65,6 +66,10 @@ def lib():
         L.heget_set_colour_stage.argtypes = [vp, C.c_int]
         L.heget_fma_probe.argtypes = [C.c_int, u64, vp, u64, C.POINTER(C.c_double), vp]
         L.heget_destroy.argtypes = [vp]
+        L.heget_static_prepare.argtypes = [vp]
+        L.heget_static_max_events.argtypes = [vp]
+        L.heget_static_max_events.restype = u64
+        L.heget_eval_me2_static.argtypes = [vp, vp, u64, vp, vp]
         L.heget_destroy.restype = None
         _lib = L
     return _lib
@@ -175,6 +180,22 @@ class Process:
         helbuf = (C.c_int8 * self.n_ext)(*[int(x) for x in hel]) if hel is not None else None
         _check(lib().heget_eval_me2(self._h, _dptr(mom, torch.float64, self.n_ext * 4 * n_events, "mom"), n_events, mode,
                                     helbuf, seed, first_event, _dptr(out, self.dtype, n_events, "out"), _stream(stream)))
+        return out
+
+    def static_prepare(self):
+        """heget_static_prepare: set-up of the entry point that allocates nothing (TABLE back end + tensor colour stage selected before)."""
+        _check(lib().heget_static_prepare(self._h))
+
+    @property
+    def static_max_events(self):
+        """heget_static_max_events: events one eval_me2_static call takes (0: not prepared)."""
+        return int(lib().heget_static_max_events(self._h))
+
+    def eval_me2_static(self, mom, out, stream=None):
+        """heget_eval_me2_static: HEL_SUM on device momenta mom[n_ext,4,E] into the caller's out[E]; no allocation anywhere in the call."""
+        n_events = mom.numel() // (self.n_ext * 4)
+        _check(lib().heget_eval_me2_static(self._h, _dptr(mom, torch.float64, self.n_ext * 4 * n_events, "mom"), n_events,
+                                           _dptr(out, self.dtype, n_events, "out"), _stream(stream)))
         return out
 
     def run_host(self, seed, n_events, first_event=0, mom_in=None, mom_out=None, weight=None, mode=HEL_SUM, hel=None,
