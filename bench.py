@@ -367,7 +367,7 @@ def run_ours(a):
                     "kernel": r["kernel"], "frac": r["frac"], "executed_frac": r["executed_frac"], "counted_tflops": r["achieved"],
                     "flops_per_event": r["flops_per_event"], "executed_flops_per_event": r["executed_flops_per_event"],
                     "regs": ci.regs_per_thread, "local_bytes": ci.local_bytes_per_thread, "threads_per_block": ci.threads_per_block,
-                    "j_in_tmem": ci.j_in_tmem, "e2e_events_per_s": mm["e2e"], "steps": a.steps if mm is m else a.sweep_steps,
+                    "j_in_tmem": ci.j_in_tmem, "warps_per_j": ci.warps_per_j, "e2e_events_per_s": mm["e2e"], "steps": a.steps if mm is m else a.sweep_steps,
                     "launch": "CUDA graph replay" if mm["graph"] else "plain", "clocks": mm["clocks"]}
 
     if rank != 0:
@@ -388,9 +388,10 @@ def run_ours(a):
                    "launch": "CUDA graph replay of the 2-kernel step" if m["graph"] else "plain stream launches",
                    "why_this_config": "BASELINE.json's metric is per process and names no single config; the headline sits on the largest one "
                                       "(C5, 7 legs, 1890 diagrams, 120 colours) in FP64; every config is in per_config"},
-        "roofline": {"bound": "alu", "kernel": "heget_eval_me2 (%s back end, %d-thread blocks, %d events/block, %d regs, %d B local, J in %s)"
+        "roofline": {"bound": "alu", "kernel": "heget_eval_me2 (%s back end, %d-thread blocks, %d events/block, %d regs, %d B local, J in %s%s)"
                                                % (roof["kernel"], info.threads_per_block, info.events_per_block, info.regs_per_thread, info.local_bytes_per_thread,
-                                                  "TMEM" if info.j_in_tmem else ("shared memory" if info.kernel == 2 else "registers/shared memory")),
+                                                  "TMEM" if info.j_in_tmem else ("shared memory" if info.kernel == 2 else "registers/shared memory"),
+                                                  ", %d producer warps + 1 updater warp per block of J" % (info.warps_per_j - 1) if info.warps_per_j > 1 else ""),
                      "achieved": roof["achieved"], "peak": roof["peak"], "unit": "TFLOP/s", "frac": roof["frac"],
                      "executed": roof["executed"], "executed_frac": roof["executed_frac"],
                      "flop_count": "achieved = flops counted by the generator for the program it emitted (FMA = 2; scheme: %s); executed = "

@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(256) k_fma_probe(T* out, unsigned long long it
 
 }  // namespace
 
-struct TabShape { int epc, jm, tm_cols, tm_wcols; size_t smem; long warps; };
+struct TabShape { int epc, jm, nsp, tm_cols, tm_wcols; size_t smem; long warps; double score; };
 enum TabElem { TE_F64 = 0, TE_F32 = 1, TE_F32X2 = 2 };      // element type of the table kernels: double, float, packed pair of floats (two events)
 struct heget_process;
 static int effective_lanes(const heget_process* p);
@@ -212,36 +212,44 @@ template <typename V> static heget_status_t upload(heget_process* p, const std::
 // threads, and for TMEM the 512 columns of an SM (a CTA allocates a power of two >= 32; the warps of a CTA that share a
 // 32-lane quadrant split the columns).  HEGET_TAB_J=smem|tmem and HEGET_TAB_EPC=n force the choice (experiments).
 template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, int regs_smem, int regs_tmem) {
-    TabShape best; best.epc = 0; best.jm = 0; best.tm_cols = 0; best.tm_wcols = 0; best.smem = 0; best.warps = -1;
+    TabShape best; best.epc = 0; best.jm = 0; best.nsp = 1; best.tm_cols = 0; best.tm_wcols = 0; best.smem = 0; best.warps = -1; best.score = -1.0;
     const char* force = getenv("HEGET_TAB_J");
     const char* force_epc = getenv("HEGET_TAB_EPC");       // slots per CTA (experiments: the block-size scan of PAPER.md:407)
+    const char* force_nsp = getenv("HEGET_TAB_NSP");       // warps per block of J (1: one warp does everything; n: n - 1 producers + 1 updater)
     for (int jm = 0; jm < 2; ++jm) {
         if (force && ((jm == 0) != (strcmp(force, "smem") == 0))) continue;
         const int regs = jm ? regs_tmem : regs_smem;
         const long reg_warps = regs > 0 ? 65536 / (((regs + 7) / 8 * 8) * 32) : 64;
-        for (int epc = 1; epc <= 8; ++epc) {
+        for (int nsp = 1; nsp <= 4; ++nsp) for (int epc = 1; epc <= 8; ++epc) {
             if (force_epc && atoi(force_epc) != epc) continue;
-            const int w = epc * d.nchunks, threads = w * 32;
-            if (threads > 256) break;
-            const size_t smem = hg::tab_smem_bytes<T>(d, epc, jm == 1) + 48;
+            if (force_nsp && atoi(force_nsp) != nsp) continue;
+            const int bwarps = epc * d.nchunks, w = bwarps * nsp, threads = w * 32;
+            if (threads > (nsp == 1 ? 256 : 480) || w > reg_warps) break;
+            if (nsp > 1 && (bwarps > 14 || (jm && bwarps % 4 != 0))) continue;      // named barrier per block of J; the warps that share a block of J in TMEM must sit in the same lane quadrant
+            const size_t smem = hg::tab_smem_bytes<T>(d, epc, jm == 1, nsp) + 48;
             if (smem > 227 * 1024) break;
             long ctas = std::min<long>(std::min<long>((long)((228 * 1024) / (smem + 1024)), 32), 2048 / threads);
             ctas = std::min<long>(ctas, reg_warps / w);
             int cols = 0, wcols = 0;
             if (jm) {
-                wcols = (int)(sizeof(T) / 4) * 2 * d.Rpad;
-                const int need = ((w + 3) / 4) * wcols;
+                wcols = (int)(sizeof(T) / 4) * 2 * (d.Rpad + 1);      // + the scratch element the padded updates go to
+                const int need = ((bwarps + 3) / 4) * wcols;
                 cols = 32; while (cols < need) cols *= 2;
                 if (cols > 512) continue;
                 ctas = std::min<long>(ctas, 512 / cols);
             }
             const long warps = ctas * w;
+            // what a shape is worth: blocks of J in flight, times what the warps of one block deliver together.  Measured (C5, g g -> 5 g,
+            // u u -> u u g g g, C4; profiles/r2_block_scan.md): one producer + updater is no faster than one warp doing both, two producers +
+            // updater deliver 1.4x, and eight independent blocks beat four specialised ones.
+            static const double gain[5] = {0.0, 1.0, 0.95, 1.4, 1.6};
+            const double score = (double)(ctas * bwarps) * gain[nsp];
             // TMEM bounds the residency but the block scheduler does not know: ask for enough shared memory that no more
             // CTAs become resident than can allocate their columns (the others would spin inside tcgen05.alloc)
             size_t ask = smem;
             if (jm && ctas > 0) ask = std::max<size_t>(smem, (size_t)(228 * 1024) / (ctas + 1) + 1024 - 1024 * 1);
             if (ask > 227 * 1024) ask = 227 * 1024;
-            if (warps > best.warps) { best.epc = epc; best.jm = jm; best.tm_cols = cols; best.tm_wcols = wcols; best.smem = ask; best.warps = warps; }
+            if (score > best.score) { best.score = score; best.epc = epc; best.jm = jm; best.nsp = nsp; best.tm_cols = cols; best.tm_wcols = wcols; best.smem = ask; best.warps = warps; }
         }
     }
     return best;
@@ -288,12 +296,30 @@ static heget_status_t table_to_device(heget_process* p) {
         auto enc8 = [&](double c, void* dst) { if (pairf) { const float f[2] = {(float)c, (float)c}; memcpy(dst, f, 8); } else memcpy(dst, &c, 8); };
         const unsigned scale = f64 ? 2u : 1u, esz = f64 ? 8u : 4u;
         const size_t ENT = f64 ? hg::tab_entry_bytes<double>() : hg::tab_entry_bytes<float>(), LT = (size_t)t.nchunks * 32;
-        const size_t npad = (size_t)t.n_entries + HG_TAB_RING + 2;
+        // launch shape first: a warp-specialised launch (nsp > 1 warps per block of J, heget_tab.cuh) walks nsp - 1 lists of records, the
+        // colour groups dealt out gpt at a time in turn; every list is padded with null records for the read-ahead of its ring
+        d.n_rows = t.n_rows; d.n_entries = t.n_entries;
+        p->tab_shape = tab_shape_of(d, p->tab_elem);
+        if (p->tab_shape.epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
+        d.nsp = p->tab_shape.nsp; d.gpt = 2;
+        const int nlists = d.nsp > 1 ? d.nsp - 1 : 1;
+        std::vector<int> seq;
+        {
+            std::vector<std::vector<int> > lists(nlists);
+            int g = 0;
+            for (int k = 0; k < t.n_entries; ++k) { lists[(g / d.gpt) % nlists].push_back(k); if ((t.b_rec[(size_t)k * 16] >> 2) & 1u) ++g; }
+            for (int l = 0; l < nlists; ++l) {
+                d.list0[l] = (int)seq.size(); d.nrec[l] = (int)lists[l].size(); d.nupd[l] = 0;
+                for (size_t i = 0; i < lists[l].size(); ++i) { seq.push_back(lists[l][i]); if ((t.b_rec[(size_t)lists[l][i] * 16] >> 3) & 15u) ++d.nupd[l]; }
+                for (int i = 0; i < HG_TAB_RING + 2; ++i) seq.push_back(-1);
+            }
+        }
+        const size_t npad = seq.size();
         std::vector<unsigned char> ent(npad * ENT, 0);
         for (size_t k = 0; k < npad; ++k) {
             uint32_t w[48]; memset(w, 0, sizeof w);
-            if (k >= (size_t)t.n_entries) { w[0] = 3u; memcpy(&ent[k * ENT], w, ENT); continue; }      // null record: no amplitude, no update
-            const uint32_t* e = &t.b_rec[k * 16];
+            if (seq[k] < 0) { w[0] = 3u; memcpy(&ent[k * ENT], w, ENT); continue; }      // null record: no amplitude, no update
+            const uint32_t* e = &t.b_rec[(size_t)seq[k] * 16];
             const unsigned kind = e[0] & 3u, reset = (e[0] >> 2) & 1u, nu = (e[0] >> 3) & 15u;
             const unsigned base[4] = {e[1] & 0xffffu, e[1] >> 16, e[2] & 0xffffu, e[2] >> 16};
             unsigned row[4], stride[4];
@@ -309,9 +335,11 @@ static heget_status_t table_to_device(heget_process* p) {
             if (f64) {
                 enc8(sgn, &w[8]);
                 for (unsigned j = 0; j < nu; ++j) { const double c = t.coef[e[6 + j] >> 16]; w[12 + 4 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 8u; enc8(c, &w[14 + 4 * j]); }
+                for (unsigned j = nu; j < (nu + 3u) / 4u * 4u; ++j) { w[12 + 4 * j] = (unsigned)t.Rpad * 2u * 32u * 8u; enc8(0.0, &w[14 + 4 * j]); }      // pads: scratch element, coefficient 0 (branch-free batches, JTmem::update)
             } else {
                 const float sf = (float)sgn; memcpy(&w[7], &sf, 4);
                 for (unsigned j = 0; j < nu; ++j) { const float c = (float)t.coef[e[6 + j] >> 16]; w[8 + 2 * j] = (e[6 + j] & 0xffffu) * 2u * 32u * 4u; memcpy(&w[9 + 2 * j], &c, 4); }      // 8 x {offset, coefficient} from byte 32
+                for (unsigned j = nu; j < (nu + 3u) / 4u * 4u; ++j) { w[8 + 2 * j] = (unsigned)t.Rpad * 2u * 32u * 4u; w[9 + 2 * j] = 0u; }
             }
             memcpy(&ent[k * ENT], w, ENT);
         }
@@ -379,8 +407,6 @@ static heget_status_t table_to_device(heget_process* p) {
         if ((st = upload(p, cf, &c)) != HEGET_OK) return st; d.coef = c;
         if (d.cstage == 1) { if ((st = upload(p, cv, &c)) != HEGET_OK) return st; d.cvals = c; }
     }
-    p->tab_shape = tab_shape_of(d, p->tab_elem);
-    if (p->tab_shape.epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
     p->tab_epc = p->tab_shape.epc;
     const int smem = (int)p->tab_shape.smem;
 #define HG_TAB_ATTR(TT) do { if (p->tab_shape.jm) CU(cudaFuncSetAttribute(hg::k_tab<TT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); else CU(cudaFuncSetAttribute(hg::k_tab<TT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); } while (0)
@@ -402,7 +428,7 @@ extern "C" {
 const char* heget_last_error(void) { return g_err; }
 uint64_t heget_launch_count(void) { return g_launches.load(); }
 #ifdef HG_TAB_TIMING
-void heget_debug_timing(unsigned long long* out, int reset) { cudaDeviceSynchronize(); cudaMemcpyFromSymbol(out, hg::g_tab_timing, 64); if (reset) { unsigned long long z[8] = {0}; cudaMemcpyToSymbol(hg::g_tab_timing, z, 64); } }
+void heget_debug_timing(unsigned long long* out, int reset) { cudaDeviceSynchronize(); cudaMemcpyFromSymbol(out, hg::g_tab_timing, 128); if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(hg::g_tab_timing, z, 128); } }
 #endif
 
 heget_status_t heget_fma_probe(heget_precision_t prec, uint64_t iters, void* d_out, uint64_t n_threads, double* flops, void* cuda_stream) {
@@ -507,7 +533,7 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
         d.Rpad = t.Rpad;
         const int elem = tab_elem_of(p->prec);
         const TabShape sh = tab_shape_of(d, elem);
-        o->events_per_block = sh.epc * (elem == TE_F32X2 ? 2 : 1); o->threads_per_block = sh.epc * t.nchunks * 32; o->j_in_tmem = sh.jm; o->packed_pairs = elem == TE_F32X2; o->colour_stage = p->colour_stage;
+        o->events_per_block = sh.epc * (elem == TE_F32X2 ? 2 : 1); o->threads_per_block = sh.epc * t.nchunks * 32 * sh.nsp; o->j_in_tmem = sh.jm; o->warps_per_j = sh.nsp; o->packed_pairs = elem == TE_F32X2; o->colour_stage = p->colour_stage;
         { std::set<long long> dv; for (size_t i = 0; i < t.colour_acc.size(); ++i) if (t.colour_acc[i] != 0.0) dv.insert((long long)llround(t.colour_acc[i] * 1e9)); o->n_color_distinct = (int)dv.size(); }
         if (have_dev) {
             cudaFuncAttributes fa;
@@ -607,7 +633,7 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         const int evpc = epc * (p->tab_elem == TE_F32X2 ? 2 : 1);       // events per CTA
         const unsigned long long blocks = (n_events + evpc - 1) / evpc;
         if (blocks > 0x7fffffffull) return fail(HEGET_EINVAL, "heget_eval_me2: n_events too large for one launch");
-        const int threads = epc * p->tdev.nchunks * 32;
+        const int threads = epc * p->tdev.nchunks * 32 * p->tdev.nsp;
         cudaStream_t s = (cudaStream_t)cuda_stream;
         const TabShape& sh = p->tab_shape;
         const double iss = 1.0 / p->sqrt_s;
@@ -794,7 +820,7 @@ heget_status_t heget_eval_me2_static(heget_process_t* p, const double* d_mom, ui
     const int epc = p->tab_epc;
     const int evpc = epc * (p->tab_elem == TE_F32X2 ? 2 : 1);
     const unsigned int blocks = (unsigned int)((n_events + evpc - 1) / evpc);
-    const int threads = epc * dev.nchunks * 32;
+    const int threads = epc * dev.nchunks * 32 * dev.nsp;
     const TabShape& sh = p->tab_shape;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const double iss = 1.0 / p->sqrt_s, oscale = p->out_scale * (double)p->tab->hel_weight;

@@ -3,7 +3,7 @@
 // the whole kernel is a few kB of instructions, so the instruction cache holds it (the straight-line kernels of the big
 // processes were instruction-fetch bound).
 //
-// Work decomposition (one CTA = EPC events x WPE warps, WPE = ceil(n_hel_eval / 32)):
+// Work decomposition (one CTA = EPC slots x WPE chunks of 32 configurations x NSP warps; a slot is one event, or two for the packed type):
 //   prologue  once per event, FP64: momenta in units of sqrt(s_hat) staged in shared memory; the momentum of every leg subset
 //             that carries a current and its 1/q^2; the external wavefunctions ixxxxx/oxxxxx/vxxxxx of both helicities
 //              written to the event's current store.
@@ -15,8 +15,13 @@
 //             amplitude = vvvxxx / ggggxx / iovxx0 of three or four stored currents, the variant of each
 //             picked by the lane's helicity bits; amplitudes of one colour group are summed in a register, then
 //             J_k += x_gk S_g (eq. 8) on the lane's column of J in shared memory.
-//   phase C   colour form  Jr^T C Jr + Ji^T C Ji (eq. 10) per lane, register-tiled over 8 rows, C streamed from
-//             global memory (L1 broadcasts); helicity sum (eq. 12) by warp shuffles; me2 = out_scale * sum.
+//   phase C   colour form  Jr^T C Jr + Ji^T C Ji (eq. 10) per lane, register-tiled over 8 rows, C streamed through
+//             the warp's ring by cp.async; helicity sum (eq. 12) by warp shuffles; me2 = out_scale * sum.
+// Warp specialisation (NSP > 1, chosen by api.cu for the processes whose J fills the tensor memory with four warps): NSP - 1 PRODUCER
+// warps walk the closing list in turn (colour groups dealt out two at a time) and one UPDATER warp applies J_k += x_gk S_g, fed
+// through mbarrier-guarded queues in shared memory, in the ORIGINAL group order -- so the additions into every J_k happen in the same
+// order as in the one-warp walk and |M|^2 is bit-identical for every NSP (tests/test_gpu_parity.py).  All NSP warps share phase A and
+// split the row tiles of phase C.
 // Current store layout: 16-byte chunks; a current with nv variants and ncomp complex components occupies
 // chunk(q, v) = base + q * nv + v, each chunk holding 2 complex (FP32) or 1 complex (FP64) -- lanes that share a variant read
 // the same chunk (multicast), lanes with different variants read neighbouring chunks (no bank conflict).
@@ -43,6 +48,12 @@ struct TabDev {
     const unsigned char* cidx;   // cstage 1: index of every coefficient of cmat in cvals
     const void* cvals;           // cstage 1: T[<= 256] distinct coefficient values
     const short* evalidx;        // [2^n_ext] helicity bits -> evaluated configuration or -1
+    // Warp specialisation (nsp > 1): nsp warps serve one (slot, chunk).  Warps 0 .. nsp - 2 are PRODUCERS: producer s walks list s of the
+    // closing records (the colour groups dealt out gpt at a time, in turn) and, at the end of a group, hands the group sum S_g and the
+    // update list to the last warp, the UPDATER, through a queue in shared memory; the updater does nothing but J_k += x_gk S_g, taking
+    // gpt groups from each queue in turn -- the original group order, so J and |M|^2 are bit-identical to the one-warp walk (nsp = 1).
+    int nsp, gpt;
+    int list0[4], nrec[4], nupd[4];   // list s: first record (index into b_ent), records, records that carry updates
 };
 
 // shared-memory bytes of one event (momenta slots + store) and of one warp's J column block
@@ -56,16 +67,24 @@ template <typename T> __host__ __device__ inline size_t tab_warp_bytes(int R) { 
 template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { return sizeof(T) == 4 ? 96 : 192; }
 #define HG_TAB_RING 16
 #define HG_TAB_MAXU 8
+#define HG_TAB_QD 4
+// one queue entry (producer -> updater): S_g of the 32 lanes, a header word (updates | last-of-group << 8) in a 16-byte line, the 8 updates of the record
+template <typename T> __host__ __device__ constexpr int tab_queue_bytes() { return 32 * 2 * (int)sizeof(T) + 16 + HG_TAB_MAXU * (sizeof(T) == 4 ? 8 : 16); }
+// one queue: mbarriers full[HG_TAB_QD], empty[HG_TAB_QD] (8 bytes each, 32 arrivals per phase: every lane of the writing / reading warp) + the entries
+#define HG_TAB_QHDR (16 * HG_TAB_QD)
+template <typename T> __host__ __device__ constexpr int tab_qblock_bytes() { return HG_TAB_QHDR + HG_TAB_QD * tab_queue_bytes<T>(); }
 template <typename T> __host__ __device__ inline size_t tab_rows_bytes(int n_rows, int nchunks) { return (((size_t)n_rows * nchunks * 32) + 15) / 16 * 16; }
-template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, bool j_in_tmem = false) {
+template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, bool j_in_tmem = false, int nsp = 1) {
     const int ev = sizeof(T) == 8 && !std::is_same<T, double>::value ? 2 : 1;      // events per slot
-    return (size_t)epc * (sizeof(double) * 4 * d.n_ext * ev + tab_event_bytes<T>(d.nK, d.store32) + (size_t)d.nchunks * ((j_in_tmem ? 0 : tab_warp_bytes<T>(d.R)) + HG_TAB_RING * tab_entry_bytes<T>()) + sizeof(double) * d.nchunks * ev)
+    return (size_t)epc * (sizeof(double) * 4 * d.n_ext * ev + tab_event_bytes<T>(d.nK, d.store32)
+                          + (size_t)d.nchunks * ((j_in_tmem ? 0 : tab_warp_bytes<T>(d.R)) + (size_t)nsp * HG_TAB_RING * tab_entry_bytes<T>() + (nsp > 1 ? (size_t)(nsp - 1) * tab_qblock_bytes<T>() : 0))
+                          + sizeof(double) * d.nchunks * 3 * ev)
            + tab_rows_bytes<T>(d.n_rows, d.nchunks);
 }
 
 #if defined(__CUDACC__)
 #ifdef HG_TAB_TIMING
-__device__ unsigned long long g_tab_timing[8];
+__device__ unsigned long long g_tab_timing[16];
 #endif
 // ---- element traits ------------------------------------------------------------------------------------------------------------
 // T = double: FP64.  T = float: FP32, one event per warp.  T = f2 (heget_dev.cuh): FP32 on packed f32x2 instructions (FFMA2 / FMUL2 /
@@ -240,11 +259,33 @@ __device__ __forceinline__ void tm_ld4(unsigned ta, unsigned& a, unsigned& b, un
 __device__ __forceinline__ void tm_st2(unsigned ta, unsigned a, unsigned b) { asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};\n" :: "r"(ta), "r"(a), "r"(b) : "memory"); }
 __device__ __forceinline__ void tm_st4(unsigned ta, unsigned a, unsigned b, unsigned c, unsigned d) { asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};\n" :: "r"(ta), "r"(a), "r"(b), "r"(c), "r"(d) : "memory"); }
 
+// producer -> updater queue of one producer (shared memory): entry n lives in slot n % QD; the producer waits on empty[slot], writes,
+// and every lane arrives on full[slot]; the updater waits on full[slot], reads, and every lane arrives on empty[slot] (mbarrier
+// arrive = release, wait = acquire: no fence instruction on either side)
+__device__ __forceinline__ void mb_init(unsigned a, unsigned count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" :: "r"(a), "r"(count) : "memory"); }
+__device__ __forceinline__ void mb_arrive(unsigned a) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" :: "r"(a) : "memory"); }
+__device__ __forceinline__ bool mb_test(unsigned a, unsigned parity) {       // one look, no waiting
+    unsigned ok;
+    asm volatile("{\n.reg .pred P1;\nmbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\nselp.u32 %0, 1, 0, P1;\n}\n" : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    return ok != 0u;
+}
+__device__ __forceinline__ void mb_wait(unsigned a, unsigned parity) {
+    asm volatile("{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}\n" :: "r"(a), "r"(parity) : "memory");
+}
+template <typename T> __device__ __forceinline__ void q_put(unsigned char* p, T re, T im) {
+    if constexpr (sizeof(T) == 4) *reinterpret_cast<float2*>(p) = make_float2(re, im); else cx_st<T>(p, mk<T>(re, im));
+}
+template <typename T> __device__ __forceinline__ void q_get(const unsigned char* p, T& re, T& im) {
+    if constexpr (sizeof(T) == 4) { const float2 v = *reinterpret_cast<const float2*>(p); re = v.x; im = v.y; } else { const cx<T> v = cx_ld<T>(p); re = v.re; im = v.im; }
+}
+// shared-window address of the queue block (0: the warp updates J itself); entries written so far; room: the slot of entry n is known to be free
+struct TabQueue { unsigned q; unsigned n; bool room; };
+
 template <typename T> struct JSmem {
     T* J;
     __device__ __forceinline__ void zero(int R) { for (int a = 0; a < 2 * R; ++a) J[a * 32] = T(0); }
     // J_k += c_j (Sr, Si) for the nu <= 8 updates of a record; off = byte offset of Re J_k in the lane's column
-    __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
+    template <int NB> __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
 #pragma unroll
         for (int j = 0; j < HG_TAB_MAXU; ++j) if (j < nu) { T* pj = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(J) + off[j]); pj[0] += c[j] * Sr; pj[32] += c[j] * Si; }
     }
@@ -256,18 +297,21 @@ template <typename T> struct JSmem {
 };
 template <typename T> struct JTmem {       // 8-byte elements: 4 columns per complex number
     unsigned ta;      // TMEM address of column 0 of this warp's block (lane field = first lane of the warp's quadrant)
-    __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st4(ta + 4 * k, 0u, 0u, 0u, 0u); tm_wait_st(); }
-    __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
+    __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8 + 1; ++k) tm_st4(ta + 4 * k, 0u, 0u, 0u, 0u); tm_wait_st(); }      // + the scratch element
+    // NB updates in flight (4 NB registers): 2 keeps the closing loop inside its register budget, the updater warp affords 4.  The batches
+    // are branch-free: the host pads every update list to a multiple of 4 with {scratch element, coefficient 0} (api.cu), so the
+    // TMEM addresses of a batch move to uniform registers together instead of one R2UR at a time between branches
+    template <int NB> __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
         tm_wait_st();
 #pragma unroll
-        for (int j0 = 0; j0 < HG_TAB_MAXU; j0 += 2) {          // two updates in flight (8 registers) keep the kernel inside its register budget
+        for (int j0 = 0; j0 < HG_TAB_MAXU; j0 += NB) {
             if (j0 >= nu) break;
-            unsigned r[2][4];
+            unsigned r[NB][4];
 #pragma unroll
-            for (int j = 0; j < 2; ++j) if (j0 + j < nu) tm_ld4(ta + (off[j0 + j] >> 7), r[j][0], r[j][1], r[j][2], r[j][3]);
+            for (int j = 0; j < NB; ++j) tm_ld4(ta + (off[j0 + j] >> 7), r[j][0], r[j][1], r[j][2], r[j][3]);
             tm_wait_ld();
 #pragma unroll
-            for (int j = 0; j < 2; ++j) if (j0 + j < nu) {
+            for (int j = 0; j < NB; ++j) {
                 const T re = el<T>::from_bits(r[j][0], r[j][1]) + c[j0 + j] * Sr, im = el<T>::from_bits(r[j][2], r[j][3]) + c[j0 + j] * Si;
                 tm_st4(ta + (off[j0 + j] >> 7), el<T>::lo(re), el<T>::hi(re), el<T>::lo(im), el<T>::hi(im));
             }
@@ -288,18 +332,18 @@ template <typename T> struct JTmem {       // 8-byte elements: 4 columns per com
 };
 template <> struct JTmem<float> {
     unsigned ta;
-    __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8; ++k) tm_st2(ta + 2 * k, 0u, 0u); tm_wait_st(); }
-    __device__ __forceinline__ void update(int nu, const unsigned* off, const float* c, float Sr, float Si) {
+    __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8 + 1; ++k) tm_st2(ta + 2 * k, 0u, 0u); tm_wait_st(); }
+    template <int NB> __device__ __forceinline__ void update(int nu, const unsigned* off, const float* c, float Sr, float Si) {
         tm_wait_st();
 #pragma unroll
-        for (int j0 = 0; j0 < HG_TAB_MAXU; j0 += 4) {
+        for (int j0 = 0; j0 < HG_TAB_MAXU; j0 += 2 * NB) {
             if (j0 >= nu) break;
-            unsigned r[4][2];
+            unsigned r[2 * NB][2];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) if (j0 + j < nu) tm_ld2(ta + (off[j0 + j] >> 7), r[j][0], r[j][1]);
+            for (int j = 0; j < 2 * NB; ++j) tm_ld2(ta + (off[j0 + j] >> 7), r[j][0], r[j][1]);
             tm_wait_ld();
 #pragma unroll
-            for (int j = 0; j < 4; ++j) if (j0 + j < nu) tm_st2(ta + (off[j0 + j] >> 7), __float_as_uint(__uint_as_float(r[j][0]) + c[j0 + j] * Sr), __float_as_uint(__uint_as_float(r[j][1]) + c[j0 + j] * Si));
+            for (int j = 0; j < 2 * NB; ++j) tm_st2(ta + (off[j0 + j] >> 7), __float_as_uint(__uint_as_float(r[j][0]) + c[j0 + j] * Sr), __float_as_uint(__uint_as_float(r[j][1]) + c[j0 + j] * Si));
         }
     }
     __device__ __forceinline__ void block8(int k0, int, float* xr, float* xi) {
@@ -313,20 +357,41 @@ template <> struct JTmem<float> {
     }
 };
 
-// the amplitude goes into its group sum; at the end of a group, J_k += x_gk S_g (eq. 8) on the lane's column
-template <typename T, typename JP> __device__ __forceinline__ void tab_apply(const cx<T>& amp, const TabCtl<T>& C, const unsigned char* ent, JP& jp, T& Sr, T& Si) {
+// the update list of a record ({byte offset of Re J_k, coefficient} x 8), from the record itself or from a queue entry
+template <typename T> __device__ __forceinline__ void tab_updates(const unsigned char* u, unsigned* off, T* c) {
+    if constexpr (sizeof(T) == 4) {
+#pragma unroll
+        for (int j = 0; j < HG_TAB_MAXU; j += 2) { const uint4 v = *reinterpret_cast<const uint4*>(u + 8 * j); off[j] = v.x; c[j] = __uint_as_float(v.y); off[j + 1] = v.z; c[j + 1] = __uint_as_float(v.w); }
+    } else {
+#pragma unroll
+        for (int j = 0; j < HG_TAB_MAXU; ++j) { const uint4 v = *reinterpret_cast<const uint4*>(u + 16 * j); off[j] = v.x; c[j] = el<T>::from_bits(v.z, v.w); }
+    }
+}
+template <typename T> __device__ __forceinline__ const unsigned char* tab_rec_updates(const unsigned char* ent) { return ent + (sizeof(T) == 4 ? 32 : 48); }
+
+// the amplitude goes into its group sum; at the end of a group, J_k += x_gk S_g (eq. 8) on the lane's column -- by this warp,
+// or (warp-specialised launch) by the updater warp, which gets S_g and the update list through the queue
+template <typename T, typename JP> __device__ __forceinline__ void tab_apply(const cx<T>& amp, const TabCtl<T>& C, const unsigned char* ent, JP& jp, T& Sr, T& Si, TabQueue& Q) {
     if ((C.ctl & 3u) != 3u) { Sr += C.sg * amp.re; Si += C.sg * amp.im; }
     const int nu = (C.ctl >> 3) & 15u;
     if (nu) {
-        unsigned off[HG_TAB_MAXU]; T c[HG_TAB_MAXU];
-        if constexpr (sizeof(T) == 4) {
-#pragma unroll
-            for (int j = 0; j < HG_TAB_MAXU; j += 2) { const uint4 u = *reinterpret_cast<const uint4*>(ent + 32 + 8 * j); off[j] = u.x; c[j] = __uint_as_float(u.y); off[j + 1] = u.z; c[j + 1] = __uint_as_float(u.w); }
+        if (Q.q) {
+            const int lane = threadIdx.x & 31;
+            const unsigned slot = Q.n & (HG_TAB_QD - 1), par = (Q.n / HG_TAB_QD) & 1u;
+            if (!Q.room) mb_wait(Q.q + 8u * HG_TAB_QD + 8u * slot, par ^ 1u);           // room: the updater has consumed entry n - QD
+            unsigned char* qe = reinterpret_cast<unsigned char*>(__cvta_shared_to_generic(Q.q + HG_TAB_QHDR + slot * tab_queue_bytes<T>()));
+            q_put<T>(qe + lane * 2 * sizeof(T), Sr, Si);
+            constexpr int UB = HG_TAB_MAXU * (sizeof(T) == 4 ? 8 : 16) / 16;      // 16-byte pieces of the update list
+            if (lane < UB) *reinterpret_cast<uint4*>(qe + 32 * 2 * sizeof(T) + 16 + 16 * lane) = *reinterpret_cast<const uint4*>(tab_rec_updates<T>(ent) + 16 * lane);
+            if (lane == UB) *reinterpret_cast<unsigned*>(qe + 32 * 2 * sizeof(T)) = (unsigned)nu | ((C.ctl & 4u) << 6);
+            mb_arrive(Q.q + 8u * slot);
+            ++Q.n;
+            Q.room = mb_test(Q.q + 8u * HG_TAB_QD + 8u * (Q.n & (HG_TAB_QD - 1)), ((Q.n / HG_TAB_QD) & 1u) ^ 1u);      // the answer arrives while the next closing is computed
         } else {
-#pragma unroll
-            for (int j = 0; j < HG_TAB_MAXU; ++j) { off[j] = *reinterpret_cast<const unsigned*>(ent + 48 + 16 * j); c[j] = cx_ld<T>(ent + 48 + 16 * j).im; }
+            unsigned off[HG_TAB_MAXU]; T c[HG_TAB_MAXU];
+            tab_updates<T>(tab_rec_updates<T>(ent), off, c);
+            jp.template update<2>(nu, off, c, Sr, Si);
         }
-        jp.update(nu, off, c, Sr, Si);
     }
     if (C.ctl & 4u) { Sr = T(0); Si = T(0); }
 }
@@ -334,7 +399,7 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_apply(con
 // One closing record from start to end.  The kind is tested ONCE and each branch loads its own operands, evaluates its vertex and
 // applies the result, so no value has to be moved into common registers where the branches meet (such moves were 12 % of the
 // instructions when the operands went through one shared structure).
-template <typename T, typename JP> __device__ __forceinline__ void tab_record(const unsigned char* ent, const unsigned char* store, const T* evK, const unsigned char* myrows, JP& jp, T& Sr, T& Si) {
+template <typename T, typename JP> __device__ __forceinline__ void tab_record(const unsigned char* ent, const unsigned char* store, const T* evK, const unsigned char* myrows, JP& jp, T& Sr, T& Si, TabQueue& Q) {
     const uint4 q0 = *reinterpret_cast<const uint4*>(ent), q1 = *reinterpret_cast<const uint4*>(ent + 16);
     const unsigned kind = q0.x & 3u;
     TabCtl<T> C; C.ctl = q0.x;
@@ -342,7 +407,7 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_record(co
     if constexpr (sizeof(T) == 4) sgc = __uint_as_float(q1.w); else sgc = cx_ld<T>(ent + 32).re;
     const unsigned fb = myrows[q0.x >> 16];
     C.sg = (fb & 1u) ? sgc : T(0); C.chi = (fb & 2u) != 0u;
-    if (kind == 3u) { tab_apply<T>(mk<T>(T(0), T(0)), C, ent, jp, Sr, Si); return; }
+    if (kind == 3u) { tab_apply<T>(mk<T>(T(0), T(0)), C, ent, jp, Sr, Si, Q); return; }
     const unsigned aa = (q0.y & 0xffffu) + myrows[q0.w & 0xffffu], ab = (q0.y >> 16) + myrows[q0.w >> 16], ac = (q0.z & 0xffffu) + myrows[q1.x & 0xffffu];
     const unsigned sa = q1.y & 0xffu, sb = (q1.y >> 8) & 0xffu, sc = (q1.y >> 16) & 0xffu;
     if (kind == 0u) {
@@ -350,35 +415,39 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_record(co
         tab_ld<T>(O.w, store, aa, sa, 4); tab_ld<T>(O.w + 4, store, ab, sb, 4); tab_ld<T>(O.w + 8, store, ac, sc, 4);
         tab_ldk4<T>(O.k, reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(evK) + (q1.z & 0xffffu)));
         tab_ldk4<T>(O.k + 4, reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(evK) + (q1.z >> 16)));
-        tab_apply<T>(tab_vvv<T>(O), C, ent, jp, Sr, Si);
+        tab_apply<T>(tab_vvv<T>(O), C, ent, jp, Sr, Si, Q);
     } else if (kind == 1u) {
         TabOps<T> O;
         const unsigned ad = (q0.z >> 16) + myrows[q1.x >> 16], sd = q1.y >> 24;
         tab_ld<T>(O.w, store, aa, sa, 4); tab_ld<T>(O.w + 4, store, ab, sb, 4); tab_ld<T>(O.w + 8, store, ac, sc, 4); tab_ld<T>(O.w + 12, store, ad, sd, 4);
-        tab_apply<T>(tab_gggg<T>(O), C, ent, jp, Sr, Si);
+        tab_apply<T>(tab_gggg<T>(O), C, ent, jp, Sr, Si, Q);
     } else {
         TabOps<T> O;
         tab_ld<T>(O.w, store, aa, sa, 2); tab_ld<T>(O.w + 2, store, ab, sb, 2); tab_ld<T>(O.w + 4, store, ac, sc, 4);
-        tab_apply<T>(tab_iov<T>(O, C.chi ? T(1) : T(-1)), C, ent, jp, Sr, Si);
+        tab_apply<T>(tab_iov<T>(O, C.chi ? T(1) : T(-1)), C, ent, jp, Sr, Si, Q);
     }
 }
 
 // JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp).
-// At most 256 threads per CTA (api.cu, tab_pick_shape).  Register budget: 136 for the 8-byte element types (at ptxas' default of
-// 128 the FP64/TMEM instantiation spilled 4 bytes), 128 for float -- zero local memory in all six instantiations.
+// Register budget: 136 for the 8-byte element types with J in TMEM (at ptxas' default of 128 the FP64/TMEM instantiation spilled 4
+// bytes), 144 with J in shared memory (the packed kernel spilled 4 bytes at 136), 128 for float -- zero local memory in all six
+// instantiations.  The launch shape (api.cu, tab_pick_shape) keeps threads x registers inside
+// the register file.
 template <typename T, int JM>
-__global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
+__global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 144 : 136) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
         const double inv_sqrt_s, const double out_scale, typename el<T>::out_t* __restrict__ me2, const int hel_mode, const int hel_fixed,
         const unsigned long long seed, const unsigned long long first_event) {
     typedef tabio<T> IO;
     extern __shared__ __align__(16) unsigned char hg_tab_smem[];
-    const int n = d.n_ext, wpe = d.nchunks, tpe = wpe * 32;
-    const int tid = threadIdx.x, el = tid / tpe, te = tid % tpe, wie = te >> 5, lane = tid & 31;
-    // carve: [pm: double 4n x epc][red: double epc x wpe][per event: evK | evI | store][per warp: J]
+    // warps of a CTA: wic = sp * (epc * wpe) + slot * wpe + chunk.  The nsp warps with the same (slot, chunk) share that block of J:
+    // wa = sp * wpe + chunk is the warp's index within its slot (nwe of them), te the thread's.
+    const int n = d.n_ext, wpe = d.nchunks, nsp = d.nsp, nwe = wpe * nsp, tpe = nwe * 32;
+    const int tid = threadIdx.x, lane = tid & 31, wic = tid >> 5, W = epc * wpe, sp = wic / W, bw = wic - sp * W, el = bw / wpe, wie = bw - el * wpe, wa = sp * wpe + wie, te = wa * 32 + lane;
+    // carve: [pm: double 4n x epc][red: double epc x wpe x 3 chains][per event: evK | evI | store][per (slot, chunk): J][per warp: ring][queues][rows]
     double* pm = reinterpret_cast<double*>(hg_tab_smem);
     double* red = pm + (size_t)4 * n * epc * hg::el<T>::EV;
     const size_t evb = tab_event_bytes<T>(d.nK, d.store32);
-    unsigned char* evbase = reinterpret_cast<unsigned char*>(red + (size_t)epc * wpe * hg::el<T>::EV);
+    unsigned char* evbase = reinterpret_cast<unsigned char*>(red + (size_t)epc * wpe * 3 * hg::el<T>::EV);
     evbase += (16 - ((size_t)(evbase - hg_tab_smem) & 15)) & 15;
     unsigned char* myev = evbase + (size_t)el * evb;
     T* evK = reinterpret_cast<T*>(myev);
@@ -387,10 +456,14 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
     unsigned char* jbase = evbase + (size_t)epc * evb;
     const size_t jwb = JM ? 0 : tab_warp_bytes<T>(d.R);
     typename std::conditional<JM == 0, JSmem<T>, JTmem<T> >::type jp;
-    if constexpr (JM == 0) jp.J = reinterpret_cast<T*>(jbase + (size_t)(el * wpe + wie) * jwb) + lane;
-    unsigned char* ring = jbase + (size_t)epc * wpe * jwb + (size_t)(el * wpe + wie) * (HG_TAB_RING * tab_entry_bytes<T>());
-    unsigned char* rows = jbase + (size_t)epc * wpe * (jwb + HG_TAB_RING * tab_entry_bytes<T>());
+    if constexpr (JM == 0) jp.J = reinterpret_cast<T*>(jbase + (size_t)bw * jwb) + lane;
+    unsigned char* ring = jbase + (size_t)epc * wpe * jwb + (size_t)wic * (HG_TAB_RING * tab_entry_bytes<T>());
+    unsigned char* qbase = jbase + (size_t)epc * wpe * jwb + (size_t)epc * nwe * (HG_TAB_RING * tab_entry_bytes<T>());      // queues: [block of J][producer]
+    const int np = nsp > 1 ? nsp - 1 : 0;
+    unsigned char* rows = qbase + (size_t)W * np * tab_qblock_bytes<T>();
     __shared__ unsigned int tm_base;
+    for (int c = tid; c < W * np * 2 * HG_TAB_QD; c += blockDim.x) mb_init((unsigned)__cvta_generic_to_shared(qbase + (size_t)(c / (2 * HG_TAB_QD)) * tab_qblock_bytes<T>() + 8 * (c % (2 * HG_TAB_QD))), 32u);
+    for (int c = tid; c < W * 3 * hg::el<T>::EV; c += blockDim.x) red[c] = 0.0;
     if constexpr (JM == 1) {
         // one warp allocates the CTA's TMEM columns and gives up the permit at once, so co-resident CTAs can allocate theirs
         if (tid < 32) {
@@ -420,8 +493,9 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
     __syncthreads();
     if constexpr (JM == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-        const int wic = tid >> 5;       // warp w of the CTA owns TMEM lanes 32 (w % 4) .. +31, and the (w / 4)-th block of tm_wcols columns
-        jp.ta = tm_base + ((unsigned)((wic & 3) * 32) << 16) + (unsigned)((wic >> 2) * tm_wcols);
+        // warp w of the CTA can reach TMEM lanes 32 (w % 4) .. +31 only; block bw of J sits in quadrant bw % 4, columns (bw / 4) tm_wcols .. ;
+        // the warps that share it have the same w % 4 because epc * wpe is a multiple of 4 whenever nsp > 1 (api.cu, tab_pick_shape)
+        jp.ta = tm_base + ((unsigned)((wic & 3) * 32) << 16) + (unsigned)((bw >> 2) * tm_wcols);
     }
     {
         typedef hg::el<T> EL;
@@ -492,7 +566,12 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
             }
         }
     }
+    if (sp == 0) {
+        jp.zero(d.R);
+        if constexpr (JM == 1) asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+    }
     __syncthreads();
+    if constexpr (JM == 1) asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
 
 #ifdef HG_TAB_TIMING
     tt1 = clock64();
@@ -500,7 +579,7 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
     // ---- phase A: off-shell currents, once per helicity variant ----------------------------------------------------------
     for (int lev = 0; lev < d.n_levels; ++lev) {
         const int b1 = (int)__ldg(d.a_level + lev + 1);
-        for (int b = (int)__ldg(d.a_level + lev) + wie; b < b1; b += wpe) {
+        for (int b = (int)__ldg(d.a_level + lev) + wa; b < b1; b += nwe) {
             const uint4 hdr = __ldg(reinterpret_cast<const uint4*>(d.a_hdr) + b);
             const uint2 od = __ldg(reinterpret_cast<const uint2*>(d.a_out) + (size_t)b * 32 + lane);
             const int nt = hdr.x & 0xff, ptype = (hdr.x >> 8) & 0xff, t0 = hdr.x >> 16;
@@ -564,18 +643,76 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
         }
         wgt = hg::el<T>::pack(wj[0], wj[EV - 1]);
     }
-    T form = T(0);
+    // The colour form is summed in THREE chains, chain c over the row tiles t = c mod 3, whatever the number of warps that share the
+    // block of J: warp sp owns the chains with c mod min(nsp, 3) == sp.  A tile's contribution is reduced over the 32 lanes (helicity
+    // sum, eq. 12, in the kernel's own precision: reading A21) and added to the chain in shared memory; the order of every addition is
+    // the same for every launch shape, and so is the last bit of |M|^2.
+    const int nown = nsp < 3 ? nsp : 3;
     if (chunk_on) {
         const int R = d.R;
-        jp.zero(R);
         T Sr = T(0), Si = T(0);
         constexpr int ENT = tab_entry_bytes<T>(), NS = HG_TAB_RING;
-        const unsigned char* gent = d.b_ent;
         const unsigned char* myrows = rows + wie * 32 + lane;
-        // the closing records stream through a per-warp ring in shared memory, six records ahead of their use (cp.async), so the
-        // latency of the table (L2) never shows
-        // refill: four records per cp.async group whenever fewer than nine are ahead; after the wait every record below
-        // issued - 4 has landed, and the loop never reads beyond issued - 6
+        if (nsp > 1 && sp == np) {
+            // ---- updater warp: J_k += x_gk S_g for the groups of every producer, gpt groups from each queue in turn ------------
+            unsigned done[3] = {0u, 0u, 0u};
+            int left = 0;
+            for (int s2 = 0; s2 < np; ++s2) left += d.nupd[s2];
+            int qi = 0, gl = d.gpt;
+            unsigned dq = 0u;
+            // the queue the next entry comes from: the current one unless it is exhausted (then the turn passes on)
+            auto pick = [&]() {
+                for (int t = 0; t < 3; ++t) {
+                    dq = qi == 0 ? done[0] : qi == 1 ? done[1] : done[2];
+                    if (dq < (unsigned)d.nupd[qi]) break;
+                    qi = qi + 1 == np ? 0 : qi + 1; gl = d.gpt;
+                }
+            };
+#ifdef HG_TAB_TIMING
+            long long uw = 0; const long long ub0 = clock64();
+#endif
+            bool ready = false;
+            if (left > 0) pick();
+            while (left > 0) {
+                const unsigned char* qb = qbase + (size_t)(bw * np + qi) * tab_qblock_bytes<T>();
+                const unsigned ca = (unsigned)__cvta_generic_to_shared(qb);
+                const unsigned slot = dq & (HG_TAB_QD - 1);
+#ifdef HG_TAB_TIMING
+                const long long tq0 = clock64();
+#endif
+                if (!ready) mb_wait(ca + 8u * slot, (dq / HG_TAB_QD) & 1u);
+#ifdef HG_TAB_TIMING
+                uw += clock64() - tq0;
+#endif
+                const unsigned char* qe = qb + HG_TAB_QHDR + slot * tab_queue_bytes<T>();
+                const unsigned hdr = *reinterpret_cast<const unsigned*>(qe + 32 * 2 * sizeof(T));
+                unsigned off[HG_TAB_MAXU]; T c[HG_TAB_MAXU];
+                q_get<T>(qe + lane * 2 * sizeof(T), Sr, Si);
+                tab_updates<T>(qe + 32 * 2 * sizeof(T) + 16, off, c);
+                mb_arrive(ca + 8u * HG_TAB_QD + 8u * slot);          // the entry is read: the producer may overwrite it
+                ++dq;
+                if (qi == 0) done[0] = dq; else if (qi == 1) done[1] = dq; else done[2] = dq;
+                --left;
+                if (hdr & 0x100u) { if (--gl == 0) { qi = qi + 1 == np ? 0 : qi + 1; gl = d.gpt; } }
+                // look at the next entry's barrier now: the answer arrives while this entry's updates go through TMEM
+                ready = false;
+                if (left > 0) {
+                    pick();
+                    ready = mb_test((unsigned)__cvta_generic_to_shared(qbase + (size_t)(bw * np + qi) * tab_qblock_bytes<T>()) + 8u * (dq & (HG_TAB_QD - 1)), (dq / HG_TAB_QD) & 1u);
+                }
+                jp.template update<sizeof(T) == 4 ? 2 : 4>((int)(hdr & 0xffu), off, c, Sr, Si);
+            }
+#ifdef HG_TAB_TIMING
+            if (lane == 0) { atomicAdd(&g_tab_timing[6], (unsigned long long)uw); atomicAdd(&g_tab_timing[7], (unsigned long long)(clock64() - ub0)); atomicAdd(&g_tab_timing[10], 1ull); }
+#endif
+        } else {
+        const int nent = d.nrec[sp];                                  // this warp's list (padded with NS null records)
+        const unsigned char* gent = d.b_ent + (size_t)d.list0[sp] * ENT;
+        TabQueue Q; Q.q = 0u; Q.n = 0u; Q.room = true;
+        if (nsp > 1) Q.q = (unsigned)__cvta_generic_to_shared(qbase + (size_t)(bw * np + sp) * tab_qblock_bytes<T>());
+        // the closing records stream through a per-warp ring of 16 records in shared memory (cp.async), so the latency of the table
+        // (L2) never shows.  refill: four records per cp.async group whenever no more than eight are ahead; after wait_group 1 every
+        // record below issued - 4 has landed, and the loop never reads beyond that
         int issued = 0;
         auto refill = [&]() {
             const unsigned char* src = gent + (size_t)issued * ENT;
@@ -588,7 +725,6 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
             asm volatile("cp.async.commit_group;\n" ::);
             issued += 4;
         };
-        const int nent = d.n_entries;                             // the table is padded with NS null records
         static_assert(HG_TAB_RING == 16, "the refill logic assumes a ring of 16 records");
         refill(); refill(); refill();
         asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp();
@@ -597,9 +733,15 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
         // evaluating two neighbouring closings of one kind together for more instruction-level parallelism (C5 FP64 9.2e5 -> 8.4e5).
         for (int k = 0; k < nent; ++k) {
             if (issued - k <= 8) { refill(); asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp(); }
-            tab_record<T>(ring + (k & (NS - 1)) * ENT, store, evK, myrows, jp, Sr, Si);
+            tab_record<T>(ring + (k & (NS - 1)) * ENT, store, evK, myrows, jp, Sr, Si, Q);
         }
         asm volatile("cp.async.wait_all;\n" ::);
+        }
+        if (nsp > 1) {          // J is complete when the updater has consumed every queue
+            if constexpr (JM == 1) { tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
+            asm volatile("bar.sync %0, %1;\n" :: "r"(1 + bw), "r"(32 * nsp) : "memory");
+            if constexpr (JM == 1) asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+        }
 #ifdef HG_TAB_TIMING
         tt3 = clock64();
 #endif
@@ -613,7 +755,7 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
             // hand J to the tensor-core colour kernel: one row per (event, configuration, re/im), Rpad columns, written 8 at a time
             typedef typename hg::el<T>::out_t OT;
             OT* X = reinterpret_cast<OT*>(d.jout);
-            for (int bb = 0; bb < ntile; ++bb) {
+            for (int bb = sp; bb < ntile; bb += nsp) {
                 T xr[8], xi[8];
                 jp.block8(8 * bb, R, xr, xi);
 #pragma unroll
@@ -645,15 +787,19 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
             asm volatile("cp.async.commit_group;\n" ::);
         };
         int buf = 0;
-        fetch(0, 0, 0);
-        for (int t = 0; t < ntile; ++t) {
+        // row tiles of this warp: those of the chains it owns, in increasing order
+        auto next_tile = [&](int t) { ++t; while (t < ntile && (t % 3) % nown != sp) ++t; return t; };
+        int t = next_tile(-1);
+        fetch(t, t, 0);
+        for (; t < ntile; t = next_tile(t)) {
             T tr[8], ti[8], dr[8], di[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) { tr[i] = T(0); ti[i] = T(0); }
             for (int bb = t; bb < ntile; ++bb) {
                 // next block: (t, bb + 1), or the first block of the next tile (nothing after the last one: an empty group)
                 const bool last_bb = bb + 1 == ntile;
-                fetch(last_bb ? t + 1 : t, last_bb ? t + 1 : bb + 1, buf ^ 1);
+                const int tn = last_bb ? next_tile(t) : t;
+                fetch(tn, last_bb ? tn : bb + 1, buf ^ 1);
                 T xr[8], xi[8];
                 jp.block8(8 * bb, R, xr, xi);
                 if (bb == t) {
@@ -694,12 +840,20 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
                 __syncwarp();
                 buf ^= 1;
             }
+            T ft = T(0);
             if (cstage == 2) {        // tiles of the Cholesky factor: t_k = sum_{b >= k} L_bk J_b, form = sum_k |t_k|^2
 #pragma unroll
-                for (int i = 0; i < 8; ++i) form += tr[i] * tr[i] + ti[i] * ti[i];
+                for (int i = 0; i < 8; ++i) ft += tr[i] * tr[i] + ti[i] * ti[i];
             } else {
 #pragma unroll
-                for (int i = 0; i < 8; ++i) form += dr[i] * tr[i] + di[i] * ti[i];
+                for (int i = 0; i < 8; ++i) ft += dr[i] * tr[i] + di[i] * ti[i];
+            }
+            ft = wgt * ft;
+#pragma unroll
+            for (int j = 0; j < EV; ++j) {
+                typename hg::el<T>::out_t a = hg::el<T>::half(ft, j);
+                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                if (lane == 0) { double* rc = red + ((size_t)(bw * 3 + t % 3) * EV + j); *rc = (double)((typename hg::el<T>::out_t)*rc + a); }
             }
         }
         asm volatile("cp.async.wait_all;\n" ::);
@@ -710,17 +864,12 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : 136) k_tab(const TabDev d, co
     tt4 = clock64();
     if (lane == 0 && chunk_on) { atomicAdd(&g_tab_timing[0], (unsigned long long)(tt1 - tt0)); atomicAdd(&g_tab_timing[1], (unsigned long long)(tt2 - tt1)); atomicAdd(&g_tab_timing[2], (unsigned long long)(tt3 - tt2)); atomicAdd(&g_tab_timing[3], (unsigned long long)(tt4 - tt3)); atomicAdd(&g_tab_timing[4], 1ull); }
 #endif
-    T acc = wgt * form;          // the helicity sum stays in the kernel's own precision (reading A21)
-#pragma unroll
-    for (int j = 0; j < EV; ++j) {
-        typename hg::el<T>::out_t a = hg::el<T>::half(acc, j);
-        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-        if (lane == 0) red[(el * wpe + wie) * EV + j] = (double)a;
-    }
     if constexpr (JM == 1) { tm_wait_ld(); tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
     __syncthreads();
     if (te < EV && e + te < n_events && d.cstage != 3) {
-        typename hg::el<T>::out_t s = 0; for (int w = 0; w < wpe; ++w) s += (typename hg::el<T>::out_t)red[(el * wpe + w) * EV + te];
+        typedef typename hg::el<T>::out_t OT;
+        OT s = 0;           // chains and chunks in a fixed order
+        for (int w = 0; w < wpe; ++w) { const double* r3 = red + (size_t)((el * wpe + w) * 3) * EV + te; s += ((OT)r3[0] + (OT)r3[EV]) + (OT)r3[2 * EV]; }
         me2[e + te] = (typename hg::el<T>::out_t)(out_scale * (double)s);
     }
     if constexpr (JM == 1) {

@@ -39,7 +39,7 @@ class Info(C.Structure):
                 ("avg_spin", C.c_double), ("avg_color", C.c_double), ("sym_factor", C.c_double),
                 ("flops_per_event", C.c_double), ("flops_per_helicity", C.c_double),
                 ("regs_per_thread", C.c_int), ("local_bytes_per_thread", C.c_int), ("threads_per_block", C.c_int), ("lanes_wide", C.c_int), ("lanes", C.c_int),
-                ("kernel", C.c_int), ("events_per_block", C.c_int), ("n_hel_computed", C.c_int), ("colour_stage", C.c_int), ("n_color_distinct", C.c_int), ("packed_pairs", C.c_int), ("j_in_tmem", C.c_int), ("flops_per_event_tensor", C.c_double)]
+                ("kernel", C.c_int), ("events_per_block", C.c_int), ("n_hel_computed", C.c_int), ("colour_stage", C.c_int), ("n_color_distinct", C.c_int), ("packed_pairs", C.c_int), ("j_in_tmem", C.c_int), ("flops_per_event_tensor", C.c_double), ("warps_per_j", C.c_int)]
 
 
 _lib = None

@@ -179,6 +179,38 @@ def test_table_kernel_matches_oracle(events, oracle_process, monkeypatch, name, 
         assert rel_err(out, other).max() <= (1e-11 if precision == "fp64" else 2e-4)
 
 
+@pytest.mark.parametrize("jmem", ["smem", "tmem"])
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("name,sqrt_s,seed,n", [("u u~ > g g g g g", 2000.0, 4, 131), ("g g > g g g g", 1500.0, 3, 197), ("u u > u u g g", 1000.0, 2, 67)])
+def test_warp_specialised_launch_is_bit_identical(events, oracle_process, monkeypatch, name, sqrt_s, seed, n, precision, jmem):
+    """Launch shapes with n > 1 warps per block of J (n - 1 producers walking the closing list in turn, one updater applying
+    J_k += x_gk S_g in the original group order; heget_tab.cuh): the same additions in the same order as the one-warp walk, so the
+    result is the same to the last bit, for J in shared memory and in tensor memory; and it matches the oracle."""
+    monkeypatch.setenv("HEGET_TAB_J", jmem)
+    mom, mom_h = events(name, sqrt_s, seed, n)
+    ref = oracle_process(name).me2(mom_h)
+    outs = {}
+    for nsp in (1, 2, 3, 4):
+        monkeypatch.setenv("HEGET_TAB_NSP", str(nsp))          # read when the handle's launch shape is chosen
+        try:
+            P = hg.Process(name, sqrt_s, precision=precision, kernel="table")
+            out = P.eval_me2(mom)
+        except hg.HegetError:
+            continue                                           # no launch shape with this many warps per J fits this process
+        assert P.info.warps_per_j == nsp and P.info.local_bytes_per_thread == 0
+        assert P.info.threads_per_block % (32 * nsp) == 0
+        outs[nsp] = out.cpu().numpy().astype(np.float64)
+        assert np.array_equal(P.eval_me2(mom).cpu().numpy().astype(np.float64), outs[nsp])      # and the same again on a second launch
+    assert 1 in outs and len(outs) >= 3, "shapes that ran: %s" % sorted(outs)
+    err = rel_err(outs[1], ref)
+    if precision == "fp64":
+        assert err.max() <= TOL64
+    else:
+        assert np.median(err) <= TOL32_MEDIAN and err.max() <= TOL32_MAX
+    for nsp, out in outs.items():
+        assert np.array_equal(out, outs[1]), "warps_per_j = %d differs from the one-warp walk" % nsp
+
+
 def test_gg_to_5g_against_explicit_colour_sum():
     """NEXT-4: g g -> g g g g g (7245 diagrams, 720 colours; the paper compiled it in 140 pieces over 90 minutes and could not run
     it).  The oracle's diagram/colour-basis tier cannot build its colour matrix (8^7 assignments x 720 traces x
