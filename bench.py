@@ -40,13 +40,13 @@ EXECUTED_FLOPS_PER_EVENT = {
     ("C1", "fp32", "straight"): 3580.0, ("C1", "fp64", "straight"): 4149.0,
     ("C2", "fp32", "straight"): 173643.0, ("C2", "fp64", "straight"): 175803.0,
     ("C3", "fp32", "straight"): 151170.0, ("C3", "fp64", "straight"): 152160.0,
-    ("C4", "fp32", "table"): 1769022.0, ("C4", "fp64", "table"): 1770157.0,
-    ("C5", "fp32", "table"): 6417107.0, ("C5", "fp64", "table"): 6375345.0,
+    ("C4", "fp32", "table"): 1775299.0, ("C4", "fp64", "table"): 1776434.0,
+    ("C5", "fp32", "table"): 6527332.0, ("C5", "fp64", "table"): 6485570.0,
 }
 METRIC = "helicity-summed |M|^2 events/sec per process on 1 B200; % of FP64/FP32 peak"
 # dram__bytes_read.sum + dram__bytes_write.sum of the |M|^2 kernel, bytes per launch, from the committed `ncu --set full` captures
 TRAFFIC = {("C2", "fp64"): 178.3e6, ("C2", "fp32"): 175.0e6,
-           ("C5", "fp64"): 60.33e6, ("C5", "fp32"): 59.67e6, ("C4", "fp64"): 219e6, ("C4", "fp32"): 212.3e6}
+           ("C5", "fp64"): 62.41e6, ("C5", "fp32"): 60.20e6, ("C4", "fp64"): 218.5e6, ("C4", "fp32"): 214.4e6}
 TRAFFIC_NOTE = {("C2", "fp64"): "profiles/r1b_ncu_c2.md (algorithmic: 168 MB in + 8 MB out)", ("C2", "fp32"): "profiles/r1b_ncu_c2.md (algorithmic: 168 MB in + 4 MB out)",
                 ("C5", "fp64"): "profiles/r2_ncu_table.md (algorithmic: 58.7 MB in + 2.1 MB out)",
                 ("C5", "fp32"): "profiles/r2_ncu_table.md (algorithmic: 58.7 MB in + 1.0 MB out)",

@@ -309,6 +309,12 @@ struct TabBuilder {
               sig[g].second = g;
           }
           std::stable_sort(sig.begin(), sig.end(), [](const std::pair<std::vector<int>, int>& a, const std::pair<std::vector<int>, int>& b) { return a.first < b.first; });
+          // ... and the sorted sequence is walked from both ends in turn (first, last, second, ...): the groups with many closings and
+          // few colour updates sit at one end and the single-closing groups with up to eight updates at the other, and a
+          // warp-specialised launch (heget_tab.cuh) wants the work of its producer warps and of its updater warp mixed evenly in time
+          { std::vector<std::pair<std::vector<int>, int> > mixed; mixed.reserve(ng);
+            for (int lo = 0, hi = ng - 1; lo <= hi; ++lo, --hi) { mixed.push_back(sig[lo]); if (hi != lo) mixed.push_back(sig[hi]); }
+            sig.swap(mixed); }
           group_order.clear();
           for (int q = 0; q < ng; ++q) {
               const int g = sig[q].second;
