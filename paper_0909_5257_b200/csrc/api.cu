@@ -302,6 +302,7 @@ static heget_status_t table_to_device(heget_process* p) {
         p->tab_shape = tab_shape_of(d, p->tab_elem);
         if (p->tab_shape.epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
         d.nsp = p->tab_shape.nsp; d.gpt = 2;
+        { const char* e = getenv("HEGET_TAB_GPT"); if (e && atoi(e) >= 1 && atoi(e) <= 64) d.gpt = atoi(e); }      // colour groups a producer takes per turn (experiments)
         const int nlists = d.nsp > 1 ? d.nsp - 1 : 1;
         std::vector<int> seq;
         {

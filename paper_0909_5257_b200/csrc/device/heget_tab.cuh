@@ -67,7 +67,9 @@ template <typename T> __host__ __device__ inline size_t tab_warp_bytes(int R) { 
 template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { return sizeof(T) == 4 ? 96 : 192; }
 #define HG_TAB_RING 16
 #define HG_TAB_MAXU 8
+#ifndef HG_TAB_QD
 #define HG_TAB_QD 4
+#endif
 // one queue entry (producer -> updater): S_g of the 32 lanes, a header word (updates | last-of-group << 8) in a 16-byte line, the 8 updates of the record
 template <typename T> __host__ __device__ constexpr int tab_queue_bytes() { return 32 * 2 * (int)sizeof(T) + 16 + HG_TAB_MAXU * (sizeof(T) == 4 ? 8 : 16); }
 // one queue: mbarriers full[HG_TAB_QD], empty[HG_TAB_QD] (8 bytes each, 32 arrivals per phase: every lane of the writing / reading warp) + the entries
@@ -279,7 +281,11 @@ template <typename T> __device__ __forceinline__ void q_get(const unsigned char*
     if constexpr (sizeof(T) == 4) { const float2 v = *reinterpret_cast<const float2*>(p); re = v.x; im = v.y; } else { const cx<T> v = cx_ld<T>(p); re = v.re; im = v.im; }
 }
 // shared-window address of the queue block (0: the warp updates J itself); entries written so far; room: the slot of entry n is known to be free
-struct TabQueue { unsigned q; unsigned n; bool room; };
+struct TabQueue { unsigned q; unsigned n; bool room;
+#ifdef HG_TAB_TIMING
+    long long wait;
+#endif
+};
 
 template <typename T> struct JSmem {
     T* J;
@@ -378,7 +384,13 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_apply(con
         if (Q.q) {
             const int lane = threadIdx.x & 31;
             const unsigned slot = Q.n & (HG_TAB_QD - 1), par = (Q.n / HG_TAB_QD) & 1u;
+#ifdef HG_TAB_TIMING
+            const long long tq0 = clock64();
+#endif
             if (!Q.room) mb_wait(Q.q + 8u * HG_TAB_QD + 8u * slot, par ^ 1u);           // room: the updater has consumed entry n - QD
+#ifdef HG_TAB_TIMING
+            Q.wait += clock64() - tq0;
+#endif
             unsigned char* qe = reinterpret_cast<unsigned char*>(__cvta_shared_to_generic(Q.q + HG_TAB_QHDR + slot * tab_queue_bytes<T>()));
             q_put<T>(qe + lane * 2 * sizeof(T), Sr, Si);
             constexpr int UB = HG_TAB_MAXU * (sizeof(T) == 4 ? 8 : 16) / 16;      // 16-byte pieces of the update list
@@ -709,6 +721,9 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 144 : 136) k_tab(co
         const int nent = d.nrec[sp];                                  // this warp's list (padded with NS null records)
         const unsigned char* gent = d.b_ent + (size_t)d.list0[sp] * ENT;
         TabQueue Q; Q.q = 0u; Q.n = 0u; Q.room = true;
+#ifdef HG_TAB_TIMING
+        Q.wait = 0; const long long pb0 = clock64();
+#endif
         if (nsp > 1) Q.q = (unsigned)__cvta_generic_to_shared(qbase + (size_t)(bw * np + sp) * tab_qblock_bytes<T>());
         // the closing records stream through a per-warp ring of 16 records in shared memory (cp.async), so the latency of the table
         // (L2) never shows.  refill: four records per cp.async group whenever no more than eight are ahead; after wait_group 1 every
@@ -736,6 +751,9 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 144 : 136) k_tab(co
             tab_record<T>(ring + (k & (NS - 1)) * ENT, store, evK, myrows, jp, Sr, Si, Q);
         }
         asm volatile("cp.async.wait_all;\n" ::);
+#ifdef HG_TAB_TIMING
+        if (lane == 0) { atomicAdd(&g_tab_timing[5], (unsigned long long)Q.wait); atomicAdd(&g_tab_timing[8], (unsigned long long)(clock64() - pb0)); atomicAdd(&g_tab_timing[9], 1ull); }
+#endif
         }
         if (nsp > 1) {          // J is complete when the updater has consumed every queue
             if constexpr (JM == 1) { tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
