@@ -211,6 +211,22 @@ def test_warp_specialised_launch_is_bit_identical(events, oracle_process, monkey
         assert np.array_equal(out, outs[1]), "warps_per_j = %d differs from the one-warp walk" % nsp
 
 
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_warp_specialised_launch_bit_identical_at_bench_scale(monkeypatch, precision):
+    """The producer/updater hand-off under load: 2^14 events of C5 through thousands of CTAs and millions of queue entries give, run after
+    run, the bits of the one-warp walk -- a lost or reordered queue entry, or a race on J, would show here."""
+    outs = {}
+    for nsp in (1, 3):
+        monkeypatch.setenv("HEGET_TAB_NSP", str(nsp))
+        P = hg.Process("u u~ > g g g g g", 2000.0, precision=precision, kernel="table")
+        mom = P.sample_momenta(7, 1 << 14)
+        runs = [P.eval_me2(mom).clone() for _ in range(3)]
+        assert P.info.warps_per_j == nsp
+        assert all(torch.equal(runs[0], r) for r in runs), "run-to-run difference with %d warps per J" % nsp
+        outs[nsp] = runs[0]
+    assert bool(torch.isfinite(outs[3]).all()) and torch.equal(outs[1], outs[3])
+
+
 def test_gg_to_5g_against_explicit_colour_sum():
     """NEXT-4: g g -> g g g g g (7245 diagrams, 720 colours; the paper compiled it in 140 pieces over 90 minutes and could not run
     it).  The oracle's diagram/colour-basis tier cannot build its colour matrix (8^7 assignments x 720 traces x
