@@ -391,7 +391,7 @@ def run_ours(a):
         "roofline": {"bound": "alu", "kernel": "heget_eval_me2 (%s back end, %d-thread blocks, %d events/block, %d regs, %d B local, J in %s%s)"
                                                % (roof["kernel"], info.threads_per_block, info.events_per_block, info.regs_per_thread, info.local_bytes_per_thread,
                                                   "TMEM" if info.j_in_tmem else ("shared memory" if info.kernel == 2 else "registers/shared memory"),
-                                                  ", %d producer warps + 1 updater warp per block of J" % (info.warps_per_j - 1) if info.warps_per_j > 1 else ""),
+                                                  ", %d warps per block of J taking turns" % info.warps_per_j if info.warps_per_j > 1 else ""),
                      "achieved": roof["achieved"], "peak": roof["peak"], "unit": "TFLOP/s", "frac": roof["frac"],
                      "executed": roof["executed"], "executed_frac": roof["executed_frac"],
                      "flop_count": "achieved = flops counted by the generator for the program it emitted (FMA = 2; scheme: %s); executed = "

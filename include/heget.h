@@ -102,8 +102,9 @@ typedef struct {
     int j_in_tmem;             /* TABLE back end: 1 if the warps keep their J in tensor memory (TMEM), 0 = shared memory */
     double flops_per_event_tensor; /* flops of the colour stage executed on the tensor pipe (0: vector pipes)        */
     int warps_per_j;           /* TABLE back end: warps that serve one block of J (32 configurations of one event, or of an event pair): 1 = one warp walks the
-                                  closing list and updates J; n > 1 = n - 1 producer warps walk the list in turn and one updater warp applies J_k += x_gk S_g
-                                  in the original group order -- the result is bit-identical for every n (heget_tab.cuh) */
+                                  closing list and updates J; n > 1 = n warps walk the list in turn (colour groups dealt out two at a time) and each applies
+                                  its J_k += x_gk S_g when its turn comes, i.e. in the original group order -- the result is bit-identical for every n
+                                  (heget_tab.cuh) */
 } heget_info_t;
 
 /* Build (or look up) the specialised kernels of one process.

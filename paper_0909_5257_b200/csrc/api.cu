@@ -211,16 +211,16 @@ template <typename V> static heget_status_t upload(heget_process* p, const std::
 // most resident warps per SM.  Bounds: shared memory, registers (regs per thread of the compiled kernel, 0 = unknown), 2048
 // threads, and for TMEM the 512 columns of an SM (a CTA allocates a power of two >= 32; the warps of a CTA that share a
 // 32-lane quadrant split the columns).  HEGET_TAB_J=smem|tmem and HEGET_TAB_EPC=n force the choice (experiments).
-template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, int regs_smem, int regs_tmem) {
+template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, const int (&kregs)[2][2]) {
     TabShape best; best.epc = 0; best.jm = 0; best.nsp = 1; best.tm_cols = 0; best.tm_wcols = 0; best.smem = 0; best.warps = -1; best.score = -1.0;
     const char* force = getenv("HEGET_TAB_J");
     const char* force_epc = getenv("HEGET_TAB_EPC");       // slots per CTA (experiments: the block-size scan of PAPER.md:407)
-    const char* force_nsp = getenv("HEGET_TAB_NSP");       // warps per block of J (1: one warp does everything; n: n - 1 producers + 1 updater)
+    const char* force_nsp = getenv("HEGET_TAB_NSP");       // warps per block of J (1: one warp does everything; n: n warps taking turns)
     for (int jm = 0; jm < 2; ++jm) {
         if (force && ((jm == 0) != (strcmp(force, "smem") == 0))) continue;
-        const int regs = jm ? regs_tmem : regs_smem;
-        const long reg_warps = regs > 0 ? 65536 / (((regs + 7) / 8 * 8) * 32) : 64;
         for (int nsp = 1; nsp <= 4; ++nsp) for (int epc = 1; epc <= 8; ++epc) {
+            const int regs = kregs[jm][nsp > 1];
+            const long reg_warps = regs > 0 ? 65536 / (((regs + 7) / 8 * 8) * 32) : 64;
             if (force_epc && atoi(force_epc) != epc) continue;
             if (force_nsp && atoi(force_nsp) != nsp) continue;
             const int bwarps = epc * d.nchunks, w = bwarps * nsp, threads = w * 32;
@@ -239,10 +239,9 @@ template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, int re
                 ctas = std::min<long>(ctas, 512 / cols);
             }
             const long warps = ctas * w;
-            // what a shape is worth: blocks of J in flight, times what the warps of one block deliver together.  Measured (C5, g g -> 5 g,
-            // u u -> u u g g g, C4; profiles/r2_block_scan.md): one producer + updater is no faster than one warp doing both, two producers +
-            // updater deliver 1.4x, and eight independent blocks beat four specialised ones.
-            static const double gain[5] = {0.0, 1.0, 0.95, 1.4, 1.6};
+            // what a shape is worth: blocks of J in flight, times what the warps of one block deliver together (measured: C5, g g -> 5 g,
+            // u u -> u u g g g, C4; profiles/r2_block_scan.md)
+            static const double gain[5] = {0.0, 1.0, 1.3, 1.6, 1.8};
             const double score = (double)(ctas * bwarps) * gain[nsp];
             // TMEM bounds the residency but the block scheduler does not know: ask for enough shared memory that no more
             // CTAs become resident than can allocate their columns (the others would spin inside tcgen05.alloc)
@@ -255,14 +254,17 @@ template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, int re
     return best;
 }
 
-template <typename T, int JM> static int tab_kernel_regs() {
+template <typename T, int JM, bool MW> static int tab_kernel_regs() {
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return 0; }
     cudaFuncAttributes fa;
-    if (cudaFuncGetAttributes(&fa, hg::k_tab<T, JM>) != cudaSuccess) { cudaGetLastError(); return 0; }
+    if (cudaFuncGetAttributes(&fa, hg::k_tab<T, JM, MW>) != cudaSuccess) { cudaGetLastError(); return 0; }
     return fa.numRegs;
 }
-template <typename T> static TabShape tab_shape_T(const hg::TabDev& d) { return tab_pick_shape<T>(d, tab_kernel_regs<T, 0>(), tab_kernel_regs<T, 1>()); }
+template <typename T> static TabShape tab_shape_T(const hg::TabDev& d) {
+    const int regs[2][2] = {{tab_kernel_regs<T, 0, false>(), tab_kernel_regs<T, 0, true>()}, {tab_kernel_regs<T, 1, false>(), tab_kernel_regs<T, 1, true>()}};      // [J in TMEM][several warps per J]
+    return tab_pick_shape<T>(d, regs);
+}
 // FP32 handles run the table program on packed f32x2 arithmetic, two events per warp (HEGET_TAB_PACK=0: scalar, one event per warp)
 static int tab_elem_of(int prec) {
     if (prec == HEGET_FP64) return TE_F64;
@@ -296,22 +298,26 @@ static heget_status_t table_to_device(heget_process* p) {
         auto enc8 = [&](double c, void* dst) { if (pairf) { const float f[2] = {(float)c, (float)c}; memcpy(dst, f, 8); } else memcpy(dst, &c, 8); };
         const unsigned scale = f64 ? 2u : 1u, esz = f64 ? 8u : 4u;
         const size_t ENT = f64 ? hg::tab_entry_bytes<double>() : hg::tab_entry_bytes<float>(), LT = (size_t)t.nchunks * 32;
-        // launch shape first: a warp-specialised launch (nsp > 1 warps per block of J, heget_tab.cuh) walks nsp - 1 lists of records, the
-        // colour groups dealt out gpt at a time in turn; every list is padded with null records for the read-ahead of its ring
+        // launch shape first: with nsp > 1 warps per block of J (heget_tab.cuh) every warp walks its own list of records, the colour groups
+        // dealt out gpt at a time in turn; every list is padded with null records for the read-ahead of its ring
         d.n_rows = t.n_rows; d.n_entries = t.n_entries;
         p->tab_shape = tab_shape_of(d, p->tab_elem);
         if (p->tab_shape.epc == 0) return fail(HEGET_EUNSUPPORTED, "process '%s': one event does not fit the shared memory of an SM", p->name.c_str());
         d.nsp = p->tab_shape.nsp; d.gpt = 2;
         { const char* e = getenv("HEGET_TAB_GPT"); if (e && atoi(e) >= 1 && atoi(e) <= 64) d.gpt = atoi(e); }      // colour groups a producer takes per turn (experiments)
-        const int nlists = d.nsp > 1 ? d.nsp - 1 : 1;
+        const int nlists = d.nsp > 1 ? d.nsp : 1;
         std::vector<int> seq;
         {
             std::vector<std::vector<int> > lists(nlists);
             int g = 0;
-            for (int k = 0; k < t.n_entries; ++k) { lists[(g / d.gpt) % nlists].push_back(k); if ((t.b_rec[(size_t)k * 16] >> 2) & 1u) ++g; }
+            for (int k = 0; k < t.n_entries; ++k) {
+                lists[(g / d.gpt) % nlists].push_back(k);
+                const uint32_t e0 = t.b_rec[(size_t)k * 16];
+                if ((e0 >> 2) & 1u) { ++g; if (((e0 >> 3) & 15u) == 0u) return fail(HEGET_EUNSUPPORTED, "process '%s': a colour group without updates", p->name.c_str()); }      // the turn passing counts groups by their last update record
+            }
             for (int l = 0; l < nlists; ++l) {
-                d.list0[l] = (int)seq.size(); d.nrec[l] = (int)lists[l].size(); d.nupd[l] = 0;
-                for (size_t i = 0; i < lists[l].size(); ++i) { seq.push_back(lists[l][i]); if ((t.b_rec[(size_t)lists[l][i] * 16] >> 3) & 15u) ++d.nupd[l]; }
+                d.list0[l] = (int)seq.size(); d.nrec[l] = (int)lists[l].size(); d.ngrp[l] = 0;
+                for (size_t i = 0; i < lists[l].size(); ++i) { seq.push_back(lists[l][i]); if ((t.b_rec[(size_t)lists[l][i] * 16] >> 2) & 1u) ++d.ngrp[l]; }
                 for (int i = 0; i < HG_TAB_RING + 2; ++i) seq.push_back(-1);
             }
         }
@@ -410,11 +416,13 @@ static heget_status_t table_to_device(heget_process* p) {
     }
     p->tab_epc = p->tab_shape.epc;
     const int smem = (int)p->tab_shape.smem;
-#define HG_TAB_ATTR(TT) do { if (p->tab_shape.jm) CU(cudaFuncSetAttribute(hg::k_tab<TT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); else CU(cudaFuncSetAttribute(hg::k_tab<TT, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); } while (0)
+#define HG_TAB_ATTR2(TT, JMV) do { if (p->tab_shape.nsp > 1) CU(cudaFuncSetAttribute(hg::k_tab<TT, JMV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); else CU(cudaFuncSetAttribute(hg::k_tab<TT, JMV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)); } while (0)
+#define HG_TAB_ATTR(TT) do { if (p->tab_shape.jm) HG_TAB_ATTR2(TT, 1); else HG_TAB_ATTR2(TT, 0); } while (0)
     if (p->tab_elem == TE_F64) HG_TAB_ATTR(double);
     else if (p->tab_elem == TE_F32) HG_TAB_ATTR(float);
     else HG_TAB_ATTR(hg::f2);
 #undef HG_TAB_ATTR
+#undef HG_TAB_ATTR2
     p->tab_on_device = true;
     return HEGET_OK;
 }
@@ -539,7 +547,7 @@ heget_status_t heget_process_info(const heget_process_t* p, heget_info_t* o) {
         if (have_dev) {
             cudaFuncAttributes fa;
             cudaError_t e;
-#define HG_TAB_FA(TT) (sh.jm ? cudaFuncGetAttributes(&fa, hg::k_tab<TT, 1>) : cudaFuncGetAttributes(&fa, hg::k_tab<TT, 0>))
+#define HG_TAB_FA(TT) (sh.jm ? (sh.nsp > 1 ? cudaFuncGetAttributes(&fa, hg::k_tab<TT, 1, true>) : cudaFuncGetAttributes(&fa, hg::k_tab<TT, 1, false>)) : (sh.nsp > 1 ? cudaFuncGetAttributes(&fa, hg::k_tab<TT, 0, true>) : cudaFuncGetAttributes(&fa, hg::k_tab<TT, 0, false>)))
             if (elem == TE_F64) e = HG_TAB_FA(double); else if (elem == TE_F32) e = HG_TAB_FA(float); else e = HG_TAB_FA(hg::f2);
 #undef HG_TAB_FA
             if (e == cudaSuccess) { o->regs_per_thread = fa.numRegs; o->local_bytes_per_thread = (int)fa.localSizeBytes; } else cudaGetLastError();
@@ -640,7 +648,7 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         const double iss = 1.0 / p->sqrt_s;
         // parity-folded helicity sum: every evaluated configuration stands for itself and its mirror image
         const double oscale = p->out_scale * (mode == HEGET_HEL_SUM ? (double)p->tab->hel_weight : 1.0);
-#define HG_TAB_LAUNCH2(TT, OT, JMV) hg::k_tab<TT, JMV><<<(unsigned int)cblocks, threads, sh.smem, s>>>(dev, epc, sh.tm_cols, sh.tm_wcols, d_mom + first, n_events, count, iss, oscale, (OT*)d_me2 + first, (int)mode, hel_fixed, seed, first_event + first)
+#define HG_TAB_LAUNCH3(TT, OT, JMV, MWV) hg::k_tab<TT, JMV, MWV><<<(unsigned int)cblocks, threads, sh.smem, s>>>(dev, epc, sh.tm_cols, sh.tm_wcols, d_mom + first, n_events, count, iss, oscale, (OT*)d_me2 + first, (int)mode, hel_fixed, seed, first_event + first)
         hg::TabDev dev = p->tdev;
         const bool tensor = dev.cstage == 3;
         unsigned long long chunk = n_events;
@@ -662,6 +670,7 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         for (unsigned long long first = 0; first < n_events; first += chunk) {
             const unsigned long long count = std::min<unsigned long long>(chunk, n_events - first);
             const unsigned long long cblocks = (count + evpc - 1) / evpc;
+#define HG_TAB_LAUNCH2(TT, OT, JMV) do { if (sh.nsp > 1) HG_TAB_LAUNCH3(TT, OT, JMV, true); else HG_TAB_LAUNCH3(TT, OT, JMV, false); } while (0)
 #define HG_TAB_LAUNCH(TT, OT) do { if (sh.jm) HG_TAB_LAUNCH2(TT, OT, 1); else HG_TAB_LAUNCH2(TT, OT, 0); } while (0)
             if (p->tab_elem == TE_F64) HG_TAB_LAUNCH(double, double);
             else if (p->tab_elem == TE_F32) HG_TAB_LAUNCH(float, float);
@@ -687,6 +696,7 @@ heget_status_t heget_eval_me2(heget_process_t* p, const double* d_mom, uint64_t 
         }
 #undef HG_TAB_LAUNCH
 #undef HG_TAB_LAUNCH2
+#undef HG_TAB_LAUNCH3
         return HEGET_OK;
     }
     const hg::ProcDesc* d = p->d;
@@ -825,13 +835,15 @@ heget_status_t heget_eval_me2_static(heget_process_t* p, const double* d_mom, ui
     const TabShape& sh = p->tab_shape;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const double iss = 1.0 / p->sqrt_s, oscale = p->out_scale * (double)p->tab->hel_weight;
-#define HG_TAB_STATIC2(TT, OT, JMV) hg::k_tab<TT, JMV><<<blocks, threads, sh.smem, s>>>(dev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, n_events, iss, oscale, (OT*)d_me2, (int)HEGET_HEL_SUM, -1, 0ull, 0ull)
+#define HG_TAB_STATIC3(TT, OT, JMV, MWV) hg::k_tab<TT, JMV, MWV><<<blocks, threads, sh.smem, s>>>(dev, epc, sh.tm_cols, sh.tm_wcols, d_mom, n_events, n_events, iss, oscale, (OT*)d_me2, (int)HEGET_HEL_SUM, -1, 0ull, 0ull)
+#define HG_TAB_STATIC2(TT, OT, JMV) do { if (sh.nsp > 1) HG_TAB_STATIC3(TT, OT, JMV, true); else HG_TAB_STATIC3(TT, OT, JMV, false); } while (0)
 #define HG_TAB_STATIC(TT, OT) do { if (sh.jm) HG_TAB_STATIC2(TT, OT, 1); else HG_TAB_STATIC2(TT, OT, 0); } while (0)
     if (p->tab_elem == TE_F64) HG_TAB_STATIC(double, double);
     else if (p->tab_elem == TE_F32) HG_TAB_STATIC(float, float);
     else HG_TAB_STATIC(hg::f2, float);
 #undef HG_TAB_STATIC
 #undef HG_TAB_STATIC2
+#undef HG_TAB_STATIC3
     CU(cudaGetLastError());
     if (p->prec == HEGET_FP64) {
         const size_t smem = (size_t)dev.Rpad * (dev.Rpad + 4) * 8;

@@ -17,11 +17,12 @@
 //             J_k += x_gk S_g (eq. 8) on the lane's column of J in shared memory.
 //   phase C   colour form  Jr^T C Jr + Ji^T C Ji (eq. 10) per lane, register-tiled over 8 rows, C streamed through
 //             the warp's ring by cp.async; helicity sum (eq. 12) by warp shuffles; me2 = out_scale * sum.
-// Warp specialisation (NSP > 1, chosen by api.cu for the processes whose J fills the tensor memory with four warps): NSP - 1 PRODUCER
-// warps walk the closing list in turn (colour groups dealt out two at a time) and one UPDATER warp applies J_k += x_gk S_g, fed
-// through mbarrier-guarded queues in shared memory, in the ORIGINAL group order -- so the additions into every J_k happen in the same
-// order as in the one-warp walk and |M|^2 is bit-identical for every NSP (tests/test_gpu_parity.py).  All NSP warps share phase A and
-// split the row tiles of phase C.
+// Several warps per block of J (NSP > 1, chosen by api.cu for the processes whose J fills the tensor memory with four warps): the
+// colour groups are dealt out to the NSP warps two at a time; every warp evaluates the closings of its groups and parks the finished
+// group sums S_g in a FIFO of its own in shared memory, and applies J_k += x_gk S_g itself when its TURN comes: the turn goes round
+// the warps in the order in which the groups were dealt (an mbarrier per warp, one phase per turn), so the additions into every J_k
+// happen in the ORIGINAL group order and |M|^2 is bit-identical for every NSP (tests/test_gpu_parity.py).  All NSP warps share
+// phase A and split the row tiles of phase C.
 // Current store layout: 16-byte chunks; a current with nv variants and ncomp complex components occupies
 // chunk(q, v) = base + q * nv + v, each chunk holding 2 complex (FP32) or 1 complex (FP64) -- lanes that share a variant read
 // the same chunk (multicast), lanes with different variants read neighbouring chunks (no bank conflict).
@@ -48,12 +49,11 @@ struct TabDev {
     const unsigned char* cidx;   // cstage 1: index of every coefficient of cmat in cvals
     const void* cvals;           // cstage 1: T[<= 256] distinct coefficient values
     const short* evalidx;        // [2^n_ext] helicity bits -> evaluated configuration or -1
-    // Warp specialisation (nsp > 1): nsp warps serve one (slot, chunk).  Warps 0 .. nsp - 2 are PRODUCERS: producer s walks list s of the
-    // closing records (the colour groups dealt out gpt at a time, in turn) and, at the end of a group, hands the group sum S_g and the
-    // update list to the last warp, the UPDATER, through a queue in shared memory; the updater does nothing but J_k += x_gk S_g, taking
-    // gpt groups from each queue in turn -- the original group order, so J and |M|^2 are bit-identical to the one-warp walk (nsp = 1).
+    // nsp > 1: nsp warps serve one (slot, chunk).  Warp s walks list s of the closing records (the colour groups dealt out gpt at a time,
+    // in turn), keeps finished group sums in its FIFO and applies them to J when its turn comes -- turn k of warp s after turn k of warp
+    // s - 1 (turn k - 1 of the last warp for s = 0): the original group order, so J and |M|^2 are bit-identical to the one-warp walk.
     int nsp, gpt;
-    int list0[4], nrec[4], nupd[4];   // list s: first record (index into b_ent), records, records that carry updates
+    int list0[4], nrec[4], ngrp[4];   // list s: first record (index into b_ent), records, colour groups
 };
 
 // shared-memory bytes of one event (momenta slots + store) and of one warp's J column block
@@ -70,16 +70,16 @@ template <typename T> __host__ __device__ constexpr int tab_entry_bytes() { retu
 #ifndef HG_TAB_QD
 #define HG_TAB_QD 4
 #endif
-// one queue entry (producer -> updater): S_g of the 32 lanes, a header word (updates | last-of-group << 8) in a 16-byte line, the 8 updates of the record
+// one FIFO entry (a finished group sum waiting for its warp's turn): S_g of the 32 lanes, a header word (updates | last-of-group << 8) in a 16-byte line, the 8 updates of the record
 template <typename T> __host__ __device__ constexpr int tab_queue_bytes() { return 32 * 2 * (int)sizeof(T) + 16 + HG_TAB_MAXU * (sizeof(T) == 4 ? 8 : 16); }
-// one queue: mbarriers full[HG_TAB_QD], empty[HG_TAB_QD] (8 bytes each, 32 arrivals per phase: every lane of the writing / reading warp) + the entries
-#define HG_TAB_QHDR (16 * HG_TAB_QD)
+// per warp: its turn mbarrier (32 arrivals per phase: every lane, when a turn of the warp is complete) in a 16-byte line + the FIFO entries
+#define HG_TAB_QHDR 16
 template <typename T> __host__ __device__ constexpr int tab_qblock_bytes() { return HG_TAB_QHDR + HG_TAB_QD * tab_queue_bytes<T>(); }
 template <typename T> __host__ __device__ inline size_t tab_rows_bytes(int n_rows, int nchunks) { return (((size_t)n_rows * nchunks * 32) + 15) / 16 * 16; }
 template <typename T> inline size_t tab_smem_bytes(const TabDev& d, int epc, bool j_in_tmem = false, int nsp = 1) {
     const int ev = sizeof(T) == 8 && !std::is_same<T, double>::value ? 2 : 1;      // events per slot
     return (size_t)epc * (sizeof(double) * 4 * d.n_ext * ev + tab_event_bytes<T>(d.nK, d.store32)
-                          + (size_t)d.nchunks * ((j_in_tmem ? 0 : tab_warp_bytes<T>(d.R)) + (size_t)nsp * HG_TAB_RING * tab_entry_bytes<T>() + (nsp > 1 ? (size_t)(nsp - 1) * tab_qblock_bytes<T>() : 0))
+                          + (size_t)d.nchunks * ((j_in_tmem ? 0 : tab_warp_bytes<T>(d.R)) + (size_t)nsp * HG_TAB_RING * tab_entry_bytes<T>() + (nsp > 1 ? (size_t)nsp * tab_qblock_bytes<T>() : 0))
                           + sizeof(double) * d.nchunks * 3 * ev)
            + tab_rows_bytes<T>(d.n_rows, d.nchunks);
 }
@@ -261,9 +261,7 @@ __device__ __forceinline__ void tm_ld4(unsigned ta, unsigned& a, unsigned& b, un
 __device__ __forceinline__ void tm_st2(unsigned ta, unsigned a, unsigned b) { asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};\n" :: "r"(ta), "r"(a), "r"(b) : "memory"); }
 __device__ __forceinline__ void tm_st4(unsigned ta, unsigned a, unsigned b, unsigned c, unsigned d) { asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};\n" :: "r"(ta), "r"(a), "r"(b), "r"(c), "r"(d) : "memory"); }
 
-// producer -> updater queue of one producer (shared memory): entry n lives in slot n % QD; the producer waits on empty[slot], writes,
-// and every lane arrives on full[slot]; the updater waits on full[slot], reads, and every lane arrives on empty[slot] (mbarrier
-// arrive = release, wait = acquire: no fence instruction on either side)
+// turn passing between the warps of one block of J: mbarrier arrive = release, test / wait = acquire (no fence instruction on either side)
 __device__ __forceinline__ void mb_init(unsigned a, unsigned count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" :: "r"(a), "r"(count) : "memory"); }
 __device__ __forceinline__ void mb_arrive(unsigned a) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" :: "r"(a) : "memory"); }
 __device__ __forceinline__ bool mb_test(unsigned a, unsigned parity) {       // one look, no waiting
@@ -280,12 +278,8 @@ template <typename T> __device__ __forceinline__ void q_put(unsigned char* p, T 
 template <typename T> __device__ __forceinline__ void q_get(const unsigned char* p, T& re, T& im) {
     if constexpr (sizeof(T) == 4) { const float2 v = *reinterpret_cast<const float2*>(p); re = v.x; im = v.y; } else { const cx<T> v = cx_ld<T>(p); re = v.re; im = v.im; }
 }
-// shared-window address of the queue block (0: the warp updates J itself); entries written so far; room: the slot of entry n is known to be free
-struct TabQueue { unsigned q; unsigned n; bool room;
-#ifdef HG_TAB_TIMING
-    long long wait;
-#endif
-};
+// shared-window address of the warp's FIFO block (0: the warp updates J at once); entries pushed so far
+struct TabQueue { unsigned q; unsigned n; };
 
 template <typename T> struct JSmem {
     T* J;
@@ -304,7 +298,7 @@ template <typename T> struct JSmem {
 template <typename T> struct JTmem {       // 8-byte elements: 4 columns per complex number
     unsigned ta;      // TMEM address of column 0 of this warp's block (lane field = first lane of the warp's quadrant)
     __device__ __forceinline__ void zero(int R) { for (int k = 0; k < (R + 7) / 8 * 8 + 1; ++k) tm_st4(ta + 4 * k, 0u, 0u, 0u, 0u); tm_wait_st(); }      // + the scratch element
-    // NB updates in flight (4 NB registers): 2 keeps the closing loop inside its register budget, the updater warp affords 4.  The batches
+    // NB updates in flight (4 NB registers): 2 keeps the closing loop inside its register budget, a FIFO drain affords 4.  The batches
     // are branch-free: the host pads every update list to a multiple of 4 with {scratch element, coefficient 0} (api.cu), so the
     // TMEM addresses of a batch move to uniform registers together instead of one R2UR at a time between branches
     template <int NB> __device__ __forceinline__ void update(int nu, const unsigned* off, const T* c, T Sr, T Si) {
@@ -376,29 +370,20 @@ template <typename T> __device__ __forceinline__ void tab_updates(const unsigned
 template <typename T> __device__ __forceinline__ const unsigned char* tab_rec_updates(const unsigned char* ent) { return ent + (sizeof(T) == 4 ? 32 : 48); }
 
 // the amplitude goes into its group sum; at the end of a group, J_k += x_gk S_g (eq. 8) on the lane's column -- by this warp,
-// or (warp-specialised launch) by the updater warp, which gets S_g and the update list through the queue
+// or (several warps per block of J) later, when the warp's turn comes: S_g and the update list wait in the warp's FIFO
 template <typename T, typename JP> __device__ __forceinline__ void tab_apply(const cx<T>& amp, const TabCtl<T>& C, const unsigned char* ent, JP& jp, T& Sr, T& Si, TabQueue& Q) {
     if ((C.ctl & 3u) != 3u) { Sr += C.sg * amp.re; Si += C.sg * amp.im; }
     const int nu = (C.ctl >> 3) & 15u;
     if (nu) {
-        if (Q.q) {
+        if (Q.q) {          // park the group sum and the record's update list in the warp's FIFO (the record loop keeps a slot free)
             const int lane = threadIdx.x & 31;
-            const unsigned slot = Q.n & (HG_TAB_QD - 1), par = (Q.n / HG_TAB_QD) & 1u;
-#ifdef HG_TAB_TIMING
-            const long long tq0 = clock64();
-#endif
-            if (!Q.room) mb_wait(Q.q + 8u * HG_TAB_QD + 8u * slot, par ^ 1u);           // room: the updater has consumed entry n - QD
-#ifdef HG_TAB_TIMING
-            Q.wait += clock64() - tq0;
-#endif
-            unsigned char* qe = reinterpret_cast<unsigned char*>(__cvta_shared_to_generic(Q.q + HG_TAB_QHDR + slot * tab_queue_bytes<T>()));
+            unsigned char* qe = reinterpret_cast<unsigned char*>(__cvta_shared_to_generic(Q.q + HG_TAB_QHDR + (Q.n & (HG_TAB_QD - 1)) * tab_queue_bytes<T>()));
             q_put<T>(qe + lane * 2 * sizeof(T), Sr, Si);
             constexpr int UB = HG_TAB_MAXU * (sizeof(T) == 4 ? 8 : 16) / 16;      // 16-byte pieces of the update list
             if (lane < UB) *reinterpret_cast<uint4*>(qe + 32 * 2 * sizeof(T) + 16 + 16 * lane) = *reinterpret_cast<const uint4*>(tab_rec_updates<T>(ent) + 16 * lane);
             if (lane == UB) *reinterpret_cast<unsigned*>(qe + 32 * 2 * sizeof(T)) = (unsigned)nu | ((C.ctl & 4u) << 6);
-            mb_arrive(Q.q + 8u * slot);
+            __syncwarp();
             ++Q.n;
-            Q.room = mb_test(Q.q + 8u * HG_TAB_QD + 8u * (Q.n & (HG_TAB_QD - 1)), ((Q.n / HG_TAB_QD) & 1u) ^ 1u);      // the answer arrives while the next closing is computed
         } else {
             unsigned off[HG_TAB_MAXU]; T c[HG_TAB_MAXU];
             tab_updates<T>(tab_rec_updates<T>(ent), off, c);
@@ -441,19 +426,20 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_record(co
 }
 
 // JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp).
+// MW: several warps per block of J (FIFOs and turn passing compiled in); the one-warp kernels carry none of it.
 // Register budget: 136 for the 8-byte element types with J in TMEM (at ptxas' default of 128 the FP64/TMEM instantiation spilled 4
-// bytes), 144 with J in shared memory (the packed kernel spilled 4 bytes at 136), 128 for float -- zero local memory in all six
-// instantiations.  The launch shape (api.cu, tab_pick_shape) keeps threads x registers inside
-// the register file.
-template <typename T, int JM>
-__global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 144 : 136) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
+// bytes), 152 with J in shared memory, 128 for float -- zero local memory in all twelve instantiations.  The launch shape (api.cu,
+// tab_pick_shape) keeps threads x registers inside the register file.
+template <typename T, int JM, bool MW>
+__global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 152 : 136) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
         const double inv_sqrt_s, const double out_scale, typename el<T>::out_t* __restrict__ me2, const int hel_mode, const int hel_fixed,
         const unsigned long long seed, const unsigned long long first_event) {
     typedef tabio<T> IO;
     extern __shared__ __align__(16) unsigned char hg_tab_smem[];
     // warps of a CTA: wic = sp * (epc * wpe) + slot * wpe + chunk.  The nsp warps with the same (slot, chunk) share that block of J:
     // wa = sp * wpe + chunk is the warp's index within its slot (nwe of them), te the thread's.
-    const int n = d.n_ext, wpe = d.nchunks, nsp = d.nsp, nwe = wpe * nsp, tpe = nwe * 32;
+    // MW: several warps per block of J (d.nsp of them); the one-warp kernel carries none of the FIFO and turn-passing code
+    const int n = d.n_ext, wpe = d.nchunks, nsp = MW ? d.nsp : 1, nwe = wpe * nsp, tpe = nwe * 32;
     const int tid = threadIdx.x, lane = tid & 31, wic = tid >> 5, W = epc * wpe, sp = wic / W, bw = wic - sp * W, el = bw / wpe, wie = bw - el * wpe, wa = sp * wpe + wie, te = wa * 32 + lane;
     // carve: [pm: double 4n x epc][red: double epc x wpe x 3 chains][per event: evK | evI | store][per (slot, chunk): J][per warp: ring][queues][rows]
     double* pm = reinterpret_cast<double*>(hg_tab_smem);
@@ -470,11 +456,11 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 144 : 136) k_tab(co
     typename std::conditional<JM == 0, JSmem<T>, JTmem<T> >::type jp;
     if constexpr (JM == 0) jp.J = reinterpret_cast<T*>(jbase + (size_t)bw * jwb) + lane;
     unsigned char* ring = jbase + (size_t)epc * wpe * jwb + (size_t)wic * (HG_TAB_RING * tab_entry_bytes<T>());
-    unsigned char* qbase = jbase + (size_t)epc * wpe * jwb + (size_t)epc * nwe * (HG_TAB_RING * tab_entry_bytes<T>());      // queues: [block of J][producer]
-    const int np = nsp > 1 ? nsp - 1 : 0;
-    unsigned char* rows = qbase + (size_t)W * np * tab_qblock_bytes<T>();
+    unsigned char* qbase = jbase + (size_t)epc * wpe * jwb + (size_t)epc * nwe * (HG_TAB_RING * tab_entry_bytes<T>());      // FIFOs: [block of J][warp]
+    const int nq = nsp > 1 ? nsp : 0;                 // FIFOs (and turn barriers) per block of J
+    unsigned char* rows = qbase + (size_t)W * nq * tab_qblock_bytes<T>();
     __shared__ unsigned int tm_base;
-    for (int c = tid; c < W * np * 2 * HG_TAB_QD; c += blockDim.x) mb_init((unsigned)__cvta_generic_to_shared(qbase + (size_t)(c / (2 * HG_TAB_QD)) * tab_qblock_bytes<T>() + 8 * (c % (2 * HG_TAB_QD))), 32u);
+    for (int c = tid; c < W * nq; c += blockDim.x) mb_init((unsigned)__cvta_generic_to_shared(qbase + (size_t)c * tab_qblock_bytes<T>()), 32u);
     for (int c = tid; c < W * 3 * hg::el<T>::EV; c += blockDim.x) red[c] = 0.0;
     if constexpr (JM == 1) {
         // one warp allocates the CTA's TMEM columns and gives up the permit at once, so co-resident CTAs can allocate theirs
@@ -665,66 +651,47 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 144 : 136) k_tab(co
         T Sr = T(0), Si = T(0);
         constexpr int ENT = tab_entry_bytes<T>(), NS = HG_TAB_RING;
         const unsigned char* myrows = rows + wie * 32 + lane;
-        if (nsp > 1 && sp == np) {
-            // ---- updater warp: J_k += x_gk S_g for the groups of every producer, gpt groups from each queue in turn ------------
-            unsigned done[3] = {0u, 0u, 0u};
-            int left = 0;
-            for (int s2 = 0; s2 < np; ++s2) left += d.nupd[s2];
-            int qi = 0, gl = d.gpt;
-            unsigned dq = 0u;
-            // the queue the next entry comes from: the current one unless it is exhausted (then the turn passes on)
-            auto pick = [&]() {
-                for (int t = 0; t < 3; ++t) {
-                    dq = qi == 0 ? done[0] : qi == 1 ? done[1] : done[2];
-                    if (dq < (unsigned)d.nupd[qi]) break;
-                    qi = qi + 1 == np ? 0 : qi + 1; gl = d.gpt;
-                }
-            };
-#ifdef HG_TAB_TIMING
-            long long uw = 0; const long long ub0 = clock64();
-#endif
-            bool ready = false;
-            if (left > 0) pick();
-            while (left > 0) {
-                const unsigned char* qb = qbase + (size_t)(bw * np + qi) * tab_qblock_bytes<T>();
-                const unsigned ca = (unsigned)__cvta_generic_to_shared(qb);
-                const unsigned slot = dq & (HG_TAB_QD - 1);
-#ifdef HG_TAB_TIMING
-                const long long tq0 = clock64();
-#endif
-                if (!ready) mb_wait(ca + 8u * slot, (dq / HG_TAB_QD) & 1u);
-#ifdef HG_TAB_TIMING
-                uw += clock64() - tq0;
-#endif
-                const unsigned char* qe = qb + HG_TAB_QHDR + slot * tab_queue_bytes<T>();
-                const unsigned hdr = *reinterpret_cast<const unsigned*>(qe + 32 * 2 * sizeof(T));
-                unsigned off[HG_TAB_MAXU]; T c[HG_TAB_MAXU];
-                q_get<T>(qe + lane * 2 * sizeof(T), Sr, Si);
-                tab_updates<T>(qe + 32 * 2 * sizeof(T) + 16, off, c);
-                mb_arrive(ca + 8u * HG_TAB_QD + 8u * slot);          // the entry is read: the producer may overwrite it
-                ++dq;
-                if (qi == 0) done[0] = dq; else if (qi == 1) done[1] = dq; else done[2] = dq;
-                --left;
-                if (hdr & 0x100u) { if (--gl == 0) { qi = qi + 1 == np ? 0 : qi + 1; gl = d.gpt; } }
-                // look at the next entry's barrier now: the answer arrives while this entry's updates go through TMEM
-                ready = false;
-                if (left > 0) {
-                    pick();
-                    ready = mb_test((unsigned)__cvta_generic_to_shared(qbase + (size_t)(bw * np + qi) * tab_qblock_bytes<T>()) + 8u * (dq & (HG_TAB_QD - 1)), (dq / HG_TAB_QD) & 1u);
-                }
-                jp.template update<sizeof(T) == 4 ? 2 : 4>((int)(hdr & 0xffu), off, c, Sr, Si);
-            }
-#ifdef HG_TAB_TIMING
-            if (lane == 0) { atomicAdd(&g_tab_timing[6], (unsigned long long)uw); atomicAdd(&g_tab_timing[7], (unsigned long long)(clock64() - ub0)); atomicAdd(&g_tab_timing[10], 1ull); }
-#endif
-        } else {
+        {
         const int nent = d.nrec[sp];                                  // this warp's list (padded with NS null records)
         const unsigned char* gent = d.b_ent + (size_t)d.list0[sp] * ENT;
-        TabQueue Q; Q.q = 0u; Q.n = 0u; Q.room = true;
-#ifdef HG_TAB_TIMING
-        Q.wait = 0; const long long pb0 = clock64();
-#endif
-        if (nsp > 1) Q.q = (unsigned)__cvta_generic_to_shared(qbase + (size_t)(bw * np + sp) * tab_qblock_bytes<T>());
+        // Several warps per block of J: finished group sums wait in this warp's FIFO until the warp's turn comes.  Turn k of warp sp (its
+        // groups k gpt .. k gpt + gpt - 1) follows turn k of warp sp - 1, or turn k - 1 of the last warp for sp = 0; a warp that completes a
+        // turn arrives on its turn barrier with all lanes (after its TMEM stores have landed), the next warp looks at that barrier.
+        TabQueue Q; Q.q = 0u; Q.n = 0u;
+        unsigned applied = 0u, turn = 0u, prev = 0u;
+        int gleft = 0;
+        bool myturn = false;
+        if constexpr (MW) {
+            Q.q = (unsigned)__cvta_generic_to_shared(qbase + (size_t)(bw * nq + sp) * tab_qblock_bytes<T>());
+            prev = (unsigned)__cvta_generic_to_shared(qbase + (size_t)(bw * nq + (sp == 0 ? nsp - 1 : sp - 1)) * tab_qblock_bytes<T>());
+            gleft = d.ngrp[sp] < d.gpt ? d.ngrp[sp] : d.gpt;
+            myturn = sp == 0;
+        }
+        // parity of the phase of the previous warp's barrier that turn `turn` of this warp waits for
+        auto turn_parity = [&]() { return (sp == 0 ? turn - 1u : turn) & 1u; };
+        // apply the parked groups for as long as it is this warp's turn
+        auto drain = [&]() {
+            if constexpr (JM == 1) asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+            while (applied != Q.n) {
+                const unsigned char* qe = reinterpret_cast<const unsigned char*>(__cvta_shared_to_generic(Q.q + HG_TAB_QHDR + (applied & (HG_TAB_QD - 1)) * tab_queue_bytes<T>()));
+                const unsigned hdr = *reinterpret_cast<const unsigned*>(qe + 32 * 2 * sizeof(T));
+                unsigned off[HG_TAB_MAXU]; T c[HG_TAB_MAXU]; T gr, gi;
+                q_get<T>(qe + lane * 2 * sizeof(T), gr, gi);
+                tab_updates<T>(qe + 32 * 2 * sizeof(T) + 16, off, c);
+                jp.template update<sizeof(T) == 4 ? 2 : 4>((int)(hdr & 0xffu), off, c, gr, gi);
+                ++applied;
+                if ((hdr & 0x100u) && --gleft == 0) {          // the turn is complete: pass it on
+                    if constexpr (JM == 1) { tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
+                    mb_arrive(Q.q);
+                    ++turn;
+                    const int rest = d.ngrp[sp] - (int)turn * d.gpt;
+                    gleft = rest < d.gpt ? rest : d.gpt;
+                    myturn = gleft > 0 && mb_test(prev, turn_parity());
+                    if (!myturn) break;
+                    if constexpr (JM == 1) asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+                }
+            }
+        };
         // the closing records stream through a per-warp ring of 16 records in shared memory (cp.async), so the latency of the table
         // (L2) never shows.  refill: four records per cp.async group whenever no more than eight are ahead; after wait_group 1 every
         // record below issued - 4 has landed, and the loop never reads beyond that
@@ -749,13 +716,21 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 144 : 136) k_tab(co
         for (int k = 0; k < nent; ++k) {
             if (issued - k <= 8) { refill(); asm volatile("cp.async.wait_group 1;\n" ::); __syncwarp(); }
             tab_record<T>(ring + (k & (NS - 1)) * ENT, store, evK, myrows, jp, Sr, Si, Q);
+            if constexpr (MW) if (Q.n != applied) {                          // parked groups: is it this warp's turn?  (the FIFO must keep a slot free for the next record)
+                if (!myturn) {
+                    if (Q.n - applied == (unsigned)HG_TAB_QD) { mb_wait(prev, turn_parity()); myturn = true; }
+                    else myturn = mb_test(prev, turn_parity());
+                }
+                if (myturn) drain();
+            }
+        }
+        if constexpr (MW) while (Q.n != applied) {         // the rest of the parked groups
+            if (!myturn) { mb_wait(prev, turn_parity()); myturn = true; }
+            drain();
         }
         asm volatile("cp.async.wait_all;\n" ::);
-#ifdef HG_TAB_TIMING
-        if (lane == 0) { atomicAdd(&g_tab_timing[5], (unsigned long long)Q.wait); atomicAdd(&g_tab_timing[8], (unsigned long long)(clock64() - pb0)); atomicAdd(&g_tab_timing[9], 1ull); }
-#endif
         }
-        if (nsp > 1) {          // J is complete when the updater has consumed every queue
+        if (nsp > 1) {          // J is complete when every warp that adds into it has had its last turn
             if constexpr (JM == 1) { tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
             asm volatile("bar.sync %0, %1;\n" :: "r"(1 + bw), "r"(32 * nsp) : "memory");
             if constexpr (JM == 1) asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");

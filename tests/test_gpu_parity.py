@@ -183,8 +183,8 @@ def test_table_kernel_matches_oracle(events, oracle_process, monkeypatch, name, 
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 @pytest.mark.parametrize("name,sqrt_s,seed,n", [("u u~ > g g g g g", 2000.0, 4, 131), ("g g > g g g g", 1500.0, 3, 197), ("u u > u u g g", 1000.0, 2, 67)])
 def test_warp_specialised_launch_is_bit_identical(events, oracle_process, monkeypatch, name, sqrt_s, seed, n, precision, jmem):
-    """Launch shapes with n > 1 warps per block of J (n - 1 producers walking the closing list in turn, one updater applying
-    J_k += x_gk S_g in the original group order; heget_tab.cuh): the same additions in the same order as the one-warp walk, so the
+    """Launch shapes with n > 1 warps per block of J (the colour groups dealt out to the n warps, each applying its J_k += x_gk S_g
+    when its turn comes, i.e. in the original group order; heget_tab.cuh): the same additions in the same order as the one-warp walk, so the
     result is the same to the last bit, for J in shared memory and in tensor memory; and it matches the oracle."""
     monkeypatch.setenv("HEGET_TAB_J", jmem)
     mom, mom_h = events(name, sqrt_s, seed, n)
@@ -213,8 +213,8 @@ def test_warp_specialised_launch_is_bit_identical(events, oracle_process, monkey
 
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 def test_warp_specialised_launch_bit_identical_at_bench_scale(monkeypatch, precision):
-    """The producer/updater hand-off under load: 2^14 events of C5 through thousands of CTAs and millions of queue entries give, run after
-    run, the bits of the one-warp walk -- a lost or reordered queue entry, or a race on J, would show here."""
+    """The turn passing between the warps of a block of J under load: 2^14 events of C5 through thousands of CTAs and millions of turns give, run after
+    run, the bits of the one-warp walk -- a lost or reordered group, or a race on J, would show here."""
     outs = {}
     for nsp in (1, 3):
         monkeypatch.setenv("HEGET_TAB_NSP", str(nsp))
