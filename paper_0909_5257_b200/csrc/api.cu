@@ -224,7 +224,7 @@ template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, const 
             if (force_epc && atoi(force_epc) != epc) continue;
             if (force_nsp && atoi(force_nsp) != nsp) continue;
             const int bwarps = epc * d.nchunks, w = bwarps * nsp, threads = w * 32;
-            if (threads > (nsp == 1 ? 256 : 480) || w > reg_warps) break;
+            if (threads > (nsp == 1 ? 256 : 512) || w > reg_warps) break;
             if (nsp > 1 && (bwarps > 14 || (jm && bwarps % 4 != 0))) continue;      // named barrier per block of J; the warps that share a block of J in TMEM must sit in the same lane quadrant
             const size_t smem = hg::tab_smem_bytes<T>(d, epc, jm == 1, nsp) + 48;
             if (smem > 227 * 1024) break;
@@ -241,7 +241,7 @@ template <typename T> static TabShape tab_pick_shape(const hg::TabDev& d, const 
             const long warps = ctas * w;
             // what a shape is worth: blocks of J in flight, times what the warps of one block deliver together (measured: C5, g g -> 5 g,
             // u u -> u u g g g, C4; profiles/r2_block_scan.md)
-            static const double gain[5] = {0.0, 1.0, 1.3, 1.6, 1.8};
+            static const double gain[5] = {0.0, 1.0, 1.2, 1.6, 1.9};
             const double score = (double)(ctas * bwarps) * gain[nsp];
             // TMEM bounds the residency but the block scheduler does not know: ask for enough shared memory that no more
             // CTAs become resident than can allocate their columns (the others would spin inside tcgen05.alloc)

@@ -427,11 +427,14 @@ template <typename T, typename JP> __device__ __forceinline__ void tab_record(co
 
 // JM = 0: J in shared memory; JM = 1: J in tensor memory (tm_cols = columns this CTA allocates, tm_wcols = columns per warp).
 // MW: several warps per block of J (FIFOs and turn passing compiled in); the one-warp kernels carry none of it.
-// Register budget: 136 for the 8-byte element types with J in TMEM (at ptxas' default of 128 the FP64/TMEM instantiation spilled 4
-// bytes), 152 with J in shared memory, 128 for float -- zero local memory in all twelve instantiations.  The launch shape (api.cu,
-// tab_pick_shape) keeps threads x registers inside the register file.
+// Register budget: the 8-byte element types get 136 with J in TMEM and one warp per J (at ptxas' default of 128 that instantiation
+// spilled 4 bytes), 128 with several warps per J (so that FOUR warps per block of J, 16 per SM, fit the register file; the kernel
+// forms its indices, its event number and its helicity weight again where phase C and the epilogue need them instead of carrying
+// them through the closing loop, which is what it took to get there without a spill), 152 with J in shared memory; float gets 128.
+// Zero local memory in all twelve instantiations.  The launch shape (api.cu, tab_pick_shape) keeps threads x registers inside the
+// register file.
 template <typename T, int JM, bool MW>
-__global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 152 : 136) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
+__global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 152 : MW ? 128 : 136) k_tab(const TabDev d, const int epc, const int tm_cols, const int tm_wcols, const double* __restrict__ mom, const unsigned long long mom_stride, const unsigned long long n_events,
         const double inv_sqrt_s, const double out_scale, typename el<T>::out_t* __restrict__ me2, const int hel_mode, const int hel_fixed,
         const unsigned long long seed, const unsigned long long first_event) {
     typedef tabio<T> IO;
@@ -623,24 +626,31 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 152 : 136) k_tab(co
     tt2 = clock64();
 #endif
     // ---- phase B: closings, one helicity configuration per lane -------------------------------------------------------------
-    const int h = wie * d.cpc + lane;
-    const bool hvalid = lane < d.cpc && h < d.NH;
-    T wgt = hvalid ? T(1) : T(0);
-    bool chunk_on = true;
-    if (hel_mode == 2) { wgt = (hvalid && h == hel_fixed) ? T(1) : T(0); chunk_on = hel_fixed >= wie * d.cpc && hel_fixed < (wie + 1) * d.cpc; }
-    else if (hel_mode == 1) {
-        double wj[2] = {0.0, 0.0}; chunk_on = false;
+    // weight of the lane's configuration in the helicity sum, and whether this chunk of configurations has anything to do.  A lambda, called
+    // before phase B (for chunk_on) and again in phase C (for the weight): nothing of it has to stay in a register through the closing loop.
+    auto hel_weight = [&](int lane_, int wie_, unsigned long long e_, bool& on) {
+        const int h = wie_ * d.cpc + lane_;
+        const bool hvalid = lane_ < d.cpc && h < d.NH;
+        T w = hvalid ? T(1) : T(0);
+        on = true;
+        if (hel_mode == 2) { w = (hvalid && h == hel_fixed) ? T(1) : T(0); on = hel_fixed >= wie_ * d.cpc && hel_fixed < (wie_ + 1) * d.cpc; }
+        else if (hel_mode == 1) {
+            double wj[2] = {0.0, 0.0}; on = false;
 #pragma unroll
-        for (int j = 0; j < EV; ++j) {
-            unsigned int r[4]; unsigned long long ej = e + j; if (ej >= n_events) ej = n_events - 1;
-            const unsigned long long ge = first_event + ej;
-            philox4x32_10((unsigned int)ge, (unsigned int)(ge >> 32), 0xffffffffu, 0u, (unsigned int)seed, (unsigned int)(seed >> 32), r);
-            const int hx = d.evalidx[r[0] >> (32 - n)];
-            wj[j] = (hvalid && h == hx) ? (double)(1 << n) : 0.0;
-            chunk_on = chunk_on || (hx >= wie * d.cpc && hx < (wie + 1) * d.cpc);
+            for (int j = 0; j < EV; ++j) {
+                unsigned int r[4]; unsigned long long ej = e_ + j; if (ej >= n_events) ej = n_events - 1;
+                const unsigned long long ge = first_event + ej;
+                philox4x32_10((unsigned int)ge, (unsigned int)(ge >> 32), 0xffffffffu, 0u, (unsigned int)seed, (unsigned int)(seed >> 32), r);
+                const int hx = d.evalidx[r[0] >> (32 - n)];
+                wj[j] = (hvalid && h == hx) ? (double)(1 << n) : 0.0;
+                on = on || (hx >= wie_ * d.cpc && hx < (wie_ + 1) * d.cpc);
+            }
+            w = hg::el<T>::pack(wj[0], wj[EV - 1]);
         }
-        wgt = hg::el<T>::pack(wj[0], wj[EV - 1]);
-    }
+        return w;
+    };
+    bool chunk_on;
+    (void)hel_weight(lane, wie, e, chunk_on);
     // The colour form is summed in THREE chains, chain c over the row tiles t = c mod 3, whatever the number of warps that share the
     // block of J: warp sp owns the chains with c mod min(nsp, 3) == sp.  A tile's contribution is reduced over the 32 lanes (helicity
     // sum, eq. 12, in the kernel's own precision: reading A21) and added to the chain in shared memory; the order of every addition is
@@ -739,6 +749,13 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 152 : 136) k_tab(co
         tt3 = clock64();
 #endif
         // ---- phase C: colour form on the accumulated basis ----------------------------------------------------------------
+        // (the thread's indices, its event and its weight are formed again here from a value the compiler cannot see through: kept in
+        // registers through the closing loop they cost the 128-register kernels a spill)
+        int tid_c = threadIdx.x; asm volatile("" : "+r"(tid_c));
+        const int lane = tid_c & 31, wic = tid_c >> 5, sp = wic / W, bw = wic - sp * W, el = bw / wpe, wie = bw - el * wpe;
+        const unsigned long long e = ((unsigned long long)blockIdx.x * epc + (unsigned long long)el) * EV;
+        double* red = reinterpret_cast<double*>(hg_tab_smem) + (size_t)4 * n * epc * EV;
+        bool on_c; const T wgt = hel_weight(lane, wie, e, on_c); (void)on_c;
         // t_a = C_aa J_a + sum_{b > a} 2 C_ab J_b for a tile of 8 rows stays in registers while J streams through (from shared
         // memory or TMEM) in blocks of 8 columns.  The 8 x 8 coefficient block of each step comes through the warp's ring
         // (free after phase B) by cp.async, one block ahead, so the latency of the matrix (L2) is hidden.
@@ -859,11 +876,15 @@ __global__ void __maxnreg__(sizeof(T) == 4 ? 128 : JM == 0 ? 152 : 136) k_tab(co
 #endif
     if constexpr (JM == 1) { tm_wait_ld(); tm_wait_st(); asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
     __syncthreads();
-    if (te < EV && e + te < n_events && d.cstage != 3) {
+    int tid_e = threadIdx.x; asm volatile("" : "+r"(tid_e));          // again: indices formed where they are used
+    const int wic_e = tid_e >> 5, sp_e = wic_e / W, bw_e = wic_e - sp_e * W, el_e = bw_e / wpe, te_e = (sp_e * wpe + bw_e - el_e * wpe) * 32 + (tid_e & 31);
+    const unsigned long long e_e = ((unsigned long long)blockIdx.x * epc + (unsigned long long)el_e) * EV;
+    const double* red_e = reinterpret_cast<const double*>(hg_tab_smem) + (size_t)4 * n * epc * EV;
+    if (te_e < EV && e_e + te_e < n_events && d.cstage != 3) {
         typedef typename hg::el<T>::out_t OT;
         OT s = 0;           // chains and chunks in a fixed order
-        for (int w = 0; w < wpe; ++w) { const double* r3 = red + (size_t)((el * wpe + w) * 3) * EV + te; s += ((OT)r3[0] + (OT)r3[EV]) + (OT)r3[2 * EV]; }
-        me2[e + te] = (typename hg::el<T>::out_t)(out_scale * (double)s);
+        for (int w = 0; w < wpe; ++w) { const double* r3 = red_e + (size_t)((el_e * wpe + w) * 3) * EV + te_e; s += ((OT)r3[0] + (OT)r3[EV]) + (OT)r3[2 * EV]; }
+        me2[e_e + te_e] = (typename hg::el<T>::out_t)(out_scale * (double)s);
     }
     if constexpr (JM == 1) {
         if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tm_base), "r"((unsigned)tm_cols) : "memory");
