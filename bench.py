@@ -46,7 +46,7 @@ EXECUTED_FLOPS_PER_EVENT = {
 METRIC = "helicity-summed |M|^2 events/sec per process on 1 B200; % of FP64/FP32 peak"
 # dram__bytes_read.sum + dram__bytes_write.sum of the |M|^2 kernel, bytes per launch, from the committed `ncu --set full` captures
 TRAFFIC = {("C2", "fp64"): 178.3e6, ("C2", "fp32"): 175.0e6,
-           ("C5", "fp64"): 61.50e6, ("C5", "fp32"): 60.35e6, ("C4", "fp64"): 217.7e6, ("C4", "fp32"): 213.1e6}
+           ("C5", "fp64"): 60.68e6, ("C5", "fp32"): 60.02e6, ("C4", "fp64"): 217.7e6, ("C4", "fp32"): 212.9e6}
 TRAFFIC_NOTE = {("C2", "fp64"): "profiles/r1b_ncu_c2.md (algorithmic: 168 MB in + 8 MB out)", ("C2", "fp32"): "profiles/r1b_ncu_c2.md (algorithmic: 168 MB in + 4 MB out)",
                 ("C5", "fp64"): "profiles/r2_ncu_table.md (algorithmic: 58.7 MB in + 2.1 MB out)",
                 ("C5", "fp32"): "profiles/r2_ncu_table.md (algorithmic: 58.7 MB in + 1.0 MB out)",
